@@ -1,0 +1,103 @@
+/* li.h -- C ABI of libli.so: the AR-aware block-sparse attention hot path of Light Interaction
+ * (arXiv 2605.31158, section 3.3) for NVIDIA B200 (sm_100a).
+ *
+ * Two operations (PAPER.md = /root/reference/PAPER.md, cited by line):
+ *   li_block_select : Eq. 9 block mean pooling of Q and of the historical K, per head;
+ *                     Eq. 10 score qbar_i . kbar_m / sqrt(d) and Top_{floor(rM)} per query block.
+ *   li_sparse_attn  : Eq. 11 context C_i = K^curr U S_i (text set T absent), then softmax
+ *                     attention of query block i over C_i ("sparse attention core").
+ * The KV context is never materialised: K/V rows are read in place from a frame-paged cache through a
+ * frame-index list  memory | temporal window | current chunk  (Fig. 2a "reconstruct the KV
+ * cache for the current chunk"; PAPER.md:146-151 describes the copies this replaces).
+ *
+ * Conventions
+ *   - Every pointer is a DEVICE pointer unless its name ends in _host.  The caller owns every buffer; the
+ *     library never allocates or frees device memory and keeps no global state besides loaded kernels.
+ *   - Calls are asynchronous on `cuda_stream` (a cudaStream_t passed as void*; NULL = default stream) and
+ *     never synchronise the device.  Host arrays are consumed before the call returns.
+ *   - Return value: LI_OK (0) or a negative LI_ERR_* code.  No C++ exception crosses this boundary.
+ *   - bf16 = IEEE bfloat16 bit patterns (uint16).  Strides are in ELEMENTS; the innermost (d) stride is 1;
+ *     every other stride must be a multiple of 8 elements and base pointers 16-byte aligned (TMA rules).
+ *   - Logical order of one call's context: history token t in [0, L_hist) is row t mod T_f of
+ *     page F[t div T_f]; chunk token u in [0, Lq) is row u mod T_f of page F[n_hist + u div T_f].
+ *     History, chunk and queries are tiled separately from their own first token into blocks of
+ *     block_k / block_k / block_q tokens; only the last block of each grid may be partial.
+ *   - There is no CPU fallback and no second backend: without a CUDA device every compute call fails
+ *     with LI_ERR_CUDA.
+ */
+#ifndef LI_H_
+#define LI_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LI_VERSION 100          /* major*100 + minor */
+#define LI_MAX_CALLS 64         /* max B per call of the library (batch of independent attention calls) */
+
+enum {
+  LI_OK = 0,
+  LI_ERR_INVALID_ARG = -1,      /* NULL pointer, non-positive size, bad stride/alignment, bad frame list */
+  LI_ERR_UNSUPPORTED = -2,      /* d not in {64,128}; block not in {64,128}; block_q != block_k; B > LI_MAX_CALLS */
+  LI_ERR_WORKSPACE   = -3,      /* workspace NULL or smaller than li_workspace_bytes() */
+  LI_ERR_CUDA        = -4       /* a CUDA runtime/driver call failed (no device, launch error, ...) */
+};
+
+typedef struct li_problem {
+  int32_t B, H, Lq, d;          /* B independent calls; Lq = n_cur_frames * frame_tokens when n_cur_frames > 0 */
+  int32_t frame_tokens;         /* T_f, tokens per cache page; multiple of 8 */
+  int32_t block_q, block_k;     /* 64 or 128; block_q == block_k */
+  int32_t n_pages;              /* pages in the cache pool */
+  const void *q;                /* bf16 Q[B,H,Lq,d] */
+  int64_t q_sb, q_sh, q_st;     /* batch / head / token strides of Q */
+  const void *k_cache;          /* bf16 [n_pages,H,T_f,d] (strides below) */
+  const void *v_cache;          /* bf16, same shape and strides as k_cache */
+  int64_t kv_sp, kv_sh, kv_st;  /* page / head / token strides of both caches */
+  const int32_t *frame_idx;     /* DEVICE int32: concatenated frame lists, logical order mem | win | cur */
+  const int32_t *frame_off_host;/* HOST int32 [B+1]: call b owns frame_idx[frame_off[b] .. frame_off[b+1]) */
+  int32_t n_cur_frames;         /* the last n_cur_frames entries of every list are the current chunk (>= 0) */
+  float   softmax_scale;        /* 0 => 1/sqrt(d) */
+} li_problem;
+
+/* Eq. 9-10.  For every call b, head h and query block i: pooled means (true cardinality
+ * in partial blocks), scores s_{i,m} = qbar_i . kbar_m / sqrt(d) in fp32, and the k_b = min(M_b, top_k_host[b])
+ * historical blocks with the largest score (ties -> lowest block index), written in ASCENDING block order.
+ *   top_k_host : HOST int32 [B]; the caller computes floor(r*M_b) in integer arithmetic.
+ *   kmax       : row pitch of sel_idx, >= max_b k_b and >= 1.
+ *   sel_idx    : int32 [B,H,Nqb,kmax]; entries beyond k_b are set to -1.
+ *   sel_cnt    : int32 [B,H,Nqb]      = k_b.
+ *   scores_opt : NULL, or fp32 [B,H,Nqb,score_pitch] receiving the scores (score_pitch >= max_b M_b).
+ *   workspace  : >= li_workspace_bytes(p, kmax) bytes, 256-byte aligned; holds qbar/kbar (fp32).
+ * Degenerate cases: M_b == 0 or k_b == 0 give sel_cnt = 0. */
+int li_block_select(const li_problem *p, const int32_t *top_k_host, int32_t kmax,
+                    int32_t *sel_idx, int32_t *sel_cnt, float *scores_opt, int32_t score_pitch,
+                    void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* Eq. 11 + attention.  Query block i of (b,h) attends ALL chunk tokens (bidirectional
+ * inside the chunk) plus the valid tokens of historical blocks sel_idx[b,h,i,0..sel_cnt[b,h,i]); the same
+ * indices address K and V.  softmax in fp32 (online), bf16 tcgen05 MMAs with fp32 accumulation.
+ *   o       : bf16 [B,H,Lq,d], contiguous.
+ *   lse_opt : NULL or fp32 [B,H,Lq]: log sum_n exp(scale * q.k_n) (natural log).
+ * An empty context (no chunk and no selected block) gives o = 0, lse = -inf.
+ * sel_idx values must lie in [0, M_b); they are not validated on the host. */
+int li_sparse_attn(const li_problem *p, const int32_t *sel_idx, const int32_t *sel_cnt, int32_t kmax,
+                   void *o, float *lse_opt, void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* Bytes of workspace both calls need for problem p (0 on invalid p). */
+size_t li_workspace_bytes(const li_problem *p, int32_t kmax);
+
+/* Number of kernel launches the two calls above issued since the last li_reset_launch_count()
+ * (bench.py's gpu_launches). */
+int64_t li_launch_count(void);
+void li_reset_launch_count(void);
+
+const char *li_strerror(int code);
+int li_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LI_H_ */

@@ -1,0 +1,195 @@
+"""paper_2605_31158_b200 -- thin ctypes binding over libli.so (include/li.h).
+
+Argument marshalling only: every step of the hot path (pooling, scoring, top-k, paged gather, attention)
+runs in the CUDA kernels of csrc/.  torch is used for device memory and streams.  There is no CPU fallback:
+if libli.so is missing or cannot be loaded, every call raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence, Tuple
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libli.so")
+
+LI_OK, LI_ERR_INVALID_ARG, LI_ERR_UNSUPPORTED, LI_ERR_WORKSPACE, LI_ERR_CUDA = 0, -1, -2, -3, -4
+LI_MAX_CALLS = 64
+
+EXPORTS = ("li_block_select", "li_sparse_attn", "li_workspace_bytes", "li_launch_count",
+           "li_reset_launch_count", "li_strerror", "li_version")
+
+
+class LiError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__(f"{where}: {strerror(code)} ({code})")
+
+
+class li_problem(ctypes.Structure):
+    """Mirror of `struct li_problem` in include/li.h."""
+    _fields_ = [
+        ("B", ctypes.c_int32), ("H", ctypes.c_int32), ("Lq", ctypes.c_int32), ("d", ctypes.c_int32),
+        ("frame_tokens", ctypes.c_int32), ("block_q", ctypes.c_int32), ("block_k", ctypes.c_int32),
+        ("n_pages", ctypes.c_int32),
+        ("q", ctypes.c_void_p), ("q_sb", ctypes.c_int64), ("q_sh", ctypes.c_int64), ("q_st", ctypes.c_int64),
+        ("k_cache", ctypes.c_void_p), ("v_cache", ctypes.c_void_p),
+        ("kv_sp", ctypes.c_int64), ("kv_sh", ctypes.c_int64), ("kv_st", ctypes.c_int64),
+        ("frame_idx", ctypes.c_void_p), ("frame_off_host", ctypes.c_void_p),
+        ("n_cur_frames", ctypes.c_int32), ("softmax_scale", ctypes.c_float),
+    ]
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Loads libli.so (never builds, never falls back)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_2605_31158_b200.build` "
+                               "(or __graft_entry__.build()); there is no CPU fallback")
+        L = ctypes.CDLL(LIB_PATH)
+        P = ctypes.POINTER(li_problem)
+        L.li_workspace_bytes.restype = ctypes.c_size_t
+        L.li_workspace_bytes.argtypes = [P, ctypes.c_int32]
+        L.li_block_select.restype = ctypes.c_int
+        L.li_block_select.argtypes = [P, ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p, ctypes.c_void_p,
+                                      ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p, ctypes.c_size_t,
+                                      ctypes.c_void_p]
+        L.li_sparse_attn.restype = ctypes.c_int
+        L.li_sparse_attn.argtypes = [P, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p,
+                                     ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p]
+        L.li_launch_count.restype = ctypes.c_int64
+        L.li_reset_launch_count.restype = None
+        L.li_strerror.restype = ctypes.c_char_p
+        L.li_strerror.argtypes = [ctypes.c_int]
+        L.li_version.restype = ctypes.c_int
+        _lib = L
+    return _lib
+
+
+def strerror(code: int) -> str:
+    return lib().li_strerror(int(code)).decode()
+
+
+def version() -> int:
+    return int(lib().li_version())
+
+
+def launch_count() -> int:
+    return int(lib().li_launch_count())
+
+
+def reset_launch_count() -> None:
+    lib().li_reset_launch_count()
+
+
+class Context:
+    """Holds one li_problem plus the host arrays it points to (kept alive for the lifetime of the object)."""
+
+    def __init__(self, q: torch.Tensor, k_cache: torch.Tensor, v_cache: torch.Tensor, frame_idx: torch.Tensor,
+                 frame_off: Sequence[int], n_cur_frames: int, block: int, softmax_scale: float = 0.0):
+        for t, name in ((q, "q"), (k_cache, "k_cache"), (v_cache, "v_cache")):
+            if t.dtype != torch.bfloat16 or not t.is_cuda or t.dim() != 4 or t.stride(-1) != 1:
+                raise ValueError(f"{name} must be a 4-D CUDA bf16 tensor with unit innermost stride")
+        if k_cache.shape != v_cache.shape or k_cache.stride() != v_cache.stride():
+            raise ValueError("k_cache and v_cache must have the same shape and strides")
+        if frame_idx.dtype != torch.int32 or not frame_idx.is_cuda or not frame_idx.is_contiguous():
+            raise ValueError("frame_idx must be a contiguous CUDA int32 tensor")
+        self.q, self.k_cache, self.v_cache, self.frame_idx = q, k_cache, v_cache, frame_idx
+        self.frame_off = np.ascontiguousarray(np.asarray(frame_off, dtype=np.int32))
+        B, H, Lq, d = q.shape
+        if len(self.frame_off) != B + 1:
+            raise ValueError("frame_off must have B+1 entries")
+        p = li_problem()
+        p.B, p.H, p.Lq, p.d = B, H, Lq, d
+        p.frame_tokens = k_cache.shape[2]
+        p.block_q = p.block_k = block
+        p.n_pages = k_cache.shape[0]
+        p.q = q.data_ptr()
+        p.q_sb, p.q_sh, p.q_st = q.stride(0), q.stride(1), q.stride(2)
+        p.k_cache, p.v_cache = k_cache.data_ptr(), v_cache.data_ptr()
+        p.kv_sp, p.kv_sh, p.kv_st = k_cache.stride(0), k_cache.stride(1), k_cache.stride(2)
+        p.frame_idx = frame_idx.data_ptr()
+        p.frame_off_host = self.frame_off.ctypes.data
+        p.n_cur_frames = n_cur_frames
+        p.softmax_scale = softmax_scale
+        self.p = p
+        self.B, self.H, self.Lq, self.d, self.block = B, H, Lq, d, block
+        self.Nqb = -(-Lq // block)
+        n_hist = (self.frame_off[1:] - self.frame_off[:-1]) - n_cur_frames
+        self.M = [-(-(int(n) * p.frame_tokens) // block) for n in n_hist]
+        self.Mmax = max(self.M) if self.M else 0
+
+    def workspace_bytes(self, kmax: int) -> int:
+        n = int(lib().li_workspace_bytes(ctypes.byref(self.p), int(kmax)))
+        if n == 0:
+            raise LiError(LI_ERR_INVALID_ARG, "li_workspace_bytes")
+        return n
+
+
+def _stream_ptr(stream: Optional[torch.cuda.Stream]) -> int:
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return int(s.cuda_stream)
+
+
+def li_workspace_bytes(ctx: Context, kmax: int) -> int:
+    return ctx.workspace_bytes(kmax)
+
+
+def li_block_select(ctx: Context, top_k: Sequence[int], kmax: int, sel_idx: torch.Tensor, sel_cnt: torch.Tensor,
+                    workspace: torch.Tensor, scores: Optional[torch.Tensor] = None,
+                    stream: Optional[torch.cuda.Stream] = None) -> None:
+    """li_block_select (include/li.h).  sel_idx int32 [B,H,Nqb,kmax], sel_cnt int32 [B,H,Nqb],
+    scores None or fp32 [B,H,Nqb,pitch]; workspace: uint8 CUDA tensor of >= li_workspace_bytes."""
+    tk = np.ascontiguousarray(np.asarray(top_k, dtype=np.int32))
+    if len(tk) != ctx.B:
+        raise ValueError("top_k must have B entries")
+    pitch = int(scores.shape[-1]) if scores is not None else 0
+    rc = lib().li_block_select(ctypes.byref(ctx.p), tk.ctypes.data, int(kmax), sel_idx.data_ptr(),
+                               sel_cnt.data_ptr(), scores.data_ptr() if scores is not None else None, pitch,
+                               workspace.data_ptr(), workspace.numel() * workspace.element_size(),
+                               _stream_ptr(stream))
+    if rc != LI_OK:
+        raise LiError(rc, "li_block_select")
+
+
+def li_sparse_attn(ctx: Context, sel_idx: torch.Tensor, sel_cnt: torch.Tensor, kmax: int, o: torch.Tensor,
+                   lse: Optional[torch.Tensor] = None, workspace: Optional[torch.Tensor] = None,
+                   stream: Optional[torch.cuda.Stream] = None) -> None:
+    """li_sparse_attn (include/li.h).  o bf16 [B,H,Lq,d] contiguous; lse None or fp32 [B,H,Lq]."""
+    rc = lib().li_sparse_attn(ctypes.byref(ctx.p), sel_idx.data_ptr(), sel_cnt.data_ptr(), int(kmax), o.data_ptr(),
+                              lse.data_ptr() if lse is not None else None,
+                              workspace.data_ptr() if workspace is not None else None,
+                              workspace.numel() * workspace.element_size() if workspace is not None else 0,
+                              _stream_ptr(stream))
+    if rc != LI_OK:
+        raise LiError(rc, "li_sparse_attn")
+
+
+class Buffers:
+    """Output/workspace tensors for one Context (allocated once by the caller, reused across calls)."""
+
+    def __init__(self, ctx: Context, kmax: int, want_scores: bool = False, want_lse: bool = True):
+        dev = ctx.q.device
+        self.kmax = int(kmax)
+        self.sel_idx = torch.empty((ctx.B, ctx.H, ctx.Nqb, self.kmax), dtype=torch.int32, device=dev)
+        self.sel_cnt = torch.empty((ctx.B, ctx.H, ctx.Nqb), dtype=torch.int32, device=dev)
+        self.scores = (torch.empty((ctx.B, ctx.H, ctx.Nqb, max(1, ctx.Mmax)), dtype=torch.float32, device=dev)
+                       if want_scores else None)
+        self.workspace = torch.empty((ctx.workspace_bytes(self.kmax),), dtype=torch.uint8, device=dev)
+        self.o = torch.empty((ctx.B, ctx.H, ctx.Lq, ctx.d), dtype=torch.bfloat16, device=dev)
+        self.lse = torch.empty((ctx.B, ctx.H, ctx.Lq), dtype=torch.float32, device=dev) if want_lse else None
+
+
+def forward(ctx: Context, top_k: Sequence[int], buf: Buffers,
+            stream: Optional[torch.cuda.Stream] = None) -> Tuple[torch.Tensor, Optional[torch.Tensor]]:
+    """One pass of the whole hot path: li_block_select then li_sparse_attn (two C-ABI calls)."""
+    li_block_select(ctx, top_k, buf.kmax, buf.sel_idx, buf.sel_cnt, buf.workspace, buf.scores, stream)
+    li_sparse_attn(ctx, buf.sel_idx, buf.sel_cnt, buf.kmax, buf.o, buf.lse, buf.workspace, stream)
+    return buf.o, buf.lse

@@ -1,0 +1,197 @@
+// li_api.cu -- the C ABI of libli.so (include/li.h): argument validation, workspace carving, TMA tensor-map
+// encoding and kernel launches.  No device allocation, no synchronisation, no global state except the
+// launch counter and the lazily resolved cuTensorMapEncodeTiled entry point.
+#include <atomic>
+#include <cmath>
+#include <cstring>
+
+#include "li_internal.h"
+
+namespace {
+
+std::atomic<int64_t> g_launches{0};
+
+using EncodeFn = CUresult (*)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                              const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                              CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeFn get_encode() {
+  static std::atomic<void *> cached{nullptr};
+  void *fn = cached.load();
+  if (fn == nullptr) {
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess ||
+        qres != cudaDriverEntryPointSuccess)
+      return nullptr;
+    cached.store(fn);
+  }
+  return reinterpret_cast<EncodeFn>(fn);
+}
+
+// bf16 tensor [n3, n2, n1, d] (innermost first: d, n1, n2, n3), strides in elements, box = 64 x rows x 1 x 1,
+// SWIZZLE_128B, out-of-bounds elements read as zero.
+bool encode_map(CUtensorMap *tm, const void *base, int d, int64_t n1, int64_t n2, int64_t n3, int64_t s1, int64_t s2,
+                int64_t s3, int box_rows) {
+  EncodeFn enc = get_encode();
+  if (enc == nullptr) return false;
+  cuuint64_t dims[4] = {(cuuint64_t)d, (cuuint64_t)n1, (cuuint64_t)n2, (cuuint64_t)n3};
+  cuuint64_t strides[3] = {(cuuint64_t)s1 * 2, (cuuint64_t)s2 * 2, (cuuint64_t)s3 * 2};
+  cuuint32_t box[4] = {64, (cuuint32_t)box_rows, 1, 1};
+  cuuint32_t estr[4] = {1, 1, 1, 1};
+  CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void *>(base), dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS;
+}
+
+inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+struct Derived {
+  int Nqb, Nc, Mmax;
+  li::BatchMeta meta;
+};
+
+// Validates p and fills the derived integers.  Returns LI_OK or an error code.
+int check_problem(const li_problem *p, Derived *dv) {
+  if (p == nullptr) return LI_ERR_INVALID_ARG;
+  if (p->B <= 0 || p->H <= 0 || p->Lq <= 0 || p->frame_tokens <= 0 || p->n_pages <= 0 || p->n_cur_frames < 0)
+    return LI_ERR_INVALID_ARG;
+  if (p->d != 64 && p->d != 128) return LI_ERR_UNSUPPORTED;
+  if (p->block_q != p->block_k || (p->block_k != 64 && p->block_k != 128)) return LI_ERR_UNSUPPORTED;
+  if (p->B > LI_MAX_CALLS) return LI_ERR_UNSUPPORTED;
+  if (p->frame_tokens % 8 != 0) return LI_ERR_INVALID_ARG;
+  if (p->q == nullptr || p->k_cache == nullptr || p->v_cache == nullptr || p->frame_idx == nullptr ||
+      p->frame_off_host == nullptr)
+    return LI_ERR_INVALID_ARG;
+  if (p->n_cur_frames > 0 && p->Lq != p->n_cur_frames * p->frame_tokens) return LI_ERR_INVALID_ARG;
+  if (p->softmax_scale < 0.f || !std::isfinite(p->softmax_scale)) return LI_ERR_INVALID_ARG;
+  const int64_t strides[6] = {p->q_sb, p->q_sh, p->q_st, p->kv_sp, p->kv_sh, p->kv_st};
+  for (int64_t s : strides)
+    if (s <= 0 || s % 8 != 0) return LI_ERR_INVALID_ARG;
+  if (p->q_st < p->d || p->kv_st < p->d) return LI_ERR_INVALID_ARG;
+  if (((uintptr_t)p->q | (uintptr_t)p->k_cache | (uintptr_t)p->v_cache) & 15u) return LI_ERR_INVALID_ARG;
+  std::memset(&dv->meta, 0, sizeof(dv->meta));
+  int mmax = 0;
+  if (p->frame_off_host[0] < 0) return LI_ERR_INVALID_ARG;
+  for (int b = 0; b < p->B; ++b) {
+    const int n = p->frame_off_host[b + 1] - p->frame_off_host[b];
+    if (n < p->n_cur_frames) return LI_ERR_INVALID_ARG;
+    const int64_t L_hist = (int64_t)(n - p->n_cur_frames) * p->frame_tokens;
+    if (L_hist + p->Lq > (int64_t)1 << 30) return LI_ERR_INVALID_ARG;
+    const int M = (int)((L_hist + p->block_k - 1) / p->block_k);
+    if (M > mmax) mmax = M;
+  }
+  for (int b = 0; b <= p->B; ++b) dv->meta.frame_off[b] = p->frame_off_host[b];
+  dv->Nqb = (p->Lq + p->block_q - 1) / p->block_q;
+  dv->Nc = (p->n_cur_frames * p->frame_tokens + p->block_k - 1) / p->block_k;
+  dv->Mmax = mmax;
+  return LI_OK;
+}
+
+size_t ws_bytes(const li_problem *p, const Derived &dv) {
+  const size_t qbar = align256((size_t)p->B * p->H * dv.Nqb * p->d * 4);
+  const size_t kbar = align256((size_t)p->B * p->H * (dv.Mmax > 0 ? dv.Mmax : 1) * p->d * 4);
+  return qbar + kbar;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t li_workspace_bytes(const li_problem *p, int32_t kmax) {
+  (void)kmax;
+  Derived dv;
+  if (check_problem(p, &dv) != LI_OK) return 0;
+  return ws_bytes(p, dv);
+}
+
+int li_block_select(const li_problem *p, const int32_t *top_k_host, int32_t kmax, int32_t *sel_idx, int32_t *sel_cnt,
+                    float *scores_opt, int32_t score_pitch, void *workspace, size_t workspace_bytes,
+                    void *cuda_stream) {
+  Derived dv;
+  int rc = check_problem(p, &dv);
+  if (rc != LI_OK) return rc;
+  if (top_k_host == nullptr || sel_idx == nullptr || sel_cnt == nullptr || kmax < 1) return LI_ERR_INVALID_ARG;
+  if (scores_opt != nullptr && score_pitch < dv.Mmax) return LI_ERR_INVALID_ARG;
+  if (workspace == nullptr || workspace_bytes < ws_bytes(p, dv) || ((uintptr_t)workspace & 255u)) return LI_ERR_WORKSPACE;
+  for (int b = 0; b < p->B; ++b) {
+    if (top_k_host[b] < 0) return LI_ERR_INVALID_ARG;
+    const int n_hist = dv.meta.frame_off[b + 1] - dv.meta.frame_off[b] - p->n_cur_frames;
+    const int M = (int)(((int64_t)n_hist * p->frame_tokens + p->block_k - 1) / p->block_k);
+    const int k = top_k_host[b] < M ? top_k_host[b] : M;
+    if (k > kmax) return LI_ERR_INVALID_ARG;
+    dv.meta.top_k[b] = k;
+  }
+  // dynamic shared memory of the score/top-k kernel: 8 rows of Mmax keys + 8 pooled query rows
+  if ((size_t)8 * dv.Mmax * 4 + (size_t)8 * p->d * 4 > 200 * 1024) return LI_ERR_UNSUPPORTED;
+
+  li::SelectParams sp;
+  std::memset(&sp, 0, sizeof(sp));
+  sp.B = p->B; sp.H = p->H; sp.Lq = p->Lq; sp.d = p->d; sp.T_f = p->frame_tokens; sp.blk = p->block_k;
+  sp.n_cur = p->n_cur_frames; sp.Nqb = dv.Nqb; sp.Mmax = dv.Mmax; sp.kmax = kmax;
+  sp.score_pitch = score_pitch;
+  sp.q = (const uint16_t *)p->q; sp.q_sb = p->q_sb; sp.q_sh = p->q_sh; sp.q_st = p->q_st;
+  sp.k_cache = (const uint16_t *)p->k_cache; sp.kv_sp = p->kv_sp; sp.kv_sh = p->kv_sh; sp.kv_st = p->kv_st;
+  sp.frame_idx = p->frame_idx;
+  sp.qbar = (float *)workspace;
+  sp.kbar = (float *)((char *)workspace + align256((size_t)p->B * p->H * dv.Nqb * p->d * 4));
+  sp.sel_idx = sel_idx; sp.sel_cnt = sel_cnt; sp.scores = scores_opt;
+  sp.inv_sqrt_d = 1.0f / std::sqrt((float)p->d);
+  int64_t n = 0;
+  const int e = li::launch_select(sp, dv.meta, (cudaStream_t)cuda_stream, &n);
+  g_launches += n;
+  return e == 0 ? LI_OK : LI_ERR_CUDA;
+}
+
+int li_sparse_attn(const li_problem *p, const int32_t *sel_idx, const int32_t *sel_cnt, int32_t kmax, void *o,
+                   float *lse_opt, void *workspace, size_t workspace_bytes, void *cuda_stream) {
+  (void)workspace; (void)workspace_bytes;   // the attention kernel needs no scratch memory
+  Derived dv;
+  int rc = check_problem(p, &dv);
+  if (rc != LI_OK) return rc;
+  if (sel_idx == nullptr || sel_cnt == nullptr || o == nullptr || kmax < 1) return LI_ERR_INVALID_ARG;
+  if ((uintptr_t)o & 15u) return LI_ERR_INVALID_ARG;
+
+  const int blk = p->block_k;
+  const int has_full = p->frame_tokens >= blk ? 1 : 0;
+  CUtensorMap tm_q, tm_kf, tm_k8, tm_vf, tm_v8;
+  bool ok = encode_map(&tm_q, p->q, p->d, p->Lq, p->H, p->B, p->q_st, p->q_sh, p->q_sb, blk);
+  ok = ok && encode_map(&tm_k8, p->k_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp, 8);
+  ok = ok && encode_map(&tm_v8, p->v_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp, 8);
+  ok = ok && encode_map(&tm_kf, p->k_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp,
+                        has_full ? blk : 8);
+  ok = ok && encode_map(&tm_vf, p->v_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp,
+                        has_full ? blk : 8);
+  if (!ok) return LI_ERR_CUDA;
+
+  li::AttnParams ap;
+  std::memset(&ap, 0, sizeof(ap));
+  ap.B = p->B; ap.H = p->H; ap.Lq = p->Lq; ap.T_f = p->frame_tokens; ap.n_cur = p->n_cur_frames;
+  ap.Nqb = dv.Nqb; ap.Nc = dv.Nc; ap.kmax = kmax; ap.has_box_full = has_full;
+  const float scale = p->softmax_scale != 0.f ? p->softmax_scale : 1.0f / std::sqrt((float)p->d);
+  ap.scale_log2 = scale * 1.4426950408889634f;
+  ap.frame_idx = p->frame_idx; ap.sel_idx = sel_idx; ap.sel_cnt = sel_cnt;
+  ap.o = (uint16_t *)o; ap.lse = lse_opt;
+  int64_t n = 0;
+  const int e = li::launch_attn(ap, dv.meta, p->d, blk, tm_q, tm_kf, tm_k8, tm_vf, tm_v8, (cudaStream_t)cuda_stream, &n);
+  g_launches += n;
+  return e == 0 ? LI_OK : LI_ERR_CUDA;
+}
+
+int64_t li_launch_count(void) { return g_launches.load(); }
+void li_reset_launch_count(void) { g_launches.store(0); }
+
+const char *li_strerror(int code) {
+  switch (code) {
+    case LI_OK: return "ok";
+    case LI_ERR_INVALID_ARG: return "invalid argument";
+    case LI_ERR_UNSUPPORTED: return "unsupported configuration";
+    case LI_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
+    case LI_ERR_CUDA: return "CUDA error";
+    default: return "unknown error";
+  }
+}
+
+int li_version(void) { return LI_VERSION; }
+
+}  // extern "C"

@@ -1,0 +1,49 @@
+// li_internal.h -- kernel parameter blocks shared by the C-ABI layer (li_api.cu) and the kernels.
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/li.h"
+
+namespace li {
+
+// Per-launch description of the batch (passed by value as a kernel parameter: no device-side metadata copy).
+struct BatchMeta {
+  int32_t frame_off[LI_MAX_CALLS + 1];  // CSR offsets into frame_idx
+  int32_t top_k[LI_MAX_CALLS];          // k_b already clamped to M_b (select only)
+};
+
+struct SelectParams {
+  int32_t B, H, Lq, d, T_f, blk, n_cur, Nqb, Mmax, kmax, score_pitch;
+  const uint16_t *q;
+  int64_t q_sb, q_sh, q_st;
+  const uint16_t *k_cache;
+  int64_t kv_sp, kv_sh, kv_st;
+  const int32_t *frame_idx;
+  float *qbar;     // [B,H,Nqb,d]
+  float *kbar;     // [B,H,Mmax,d]
+  int32_t *sel_idx;
+  int32_t *sel_cnt;
+  float *scores;   // optional
+  float inv_sqrt_d;
+};
+
+struct AttnParams {
+  int32_t B, H, Lq, T_f, n_cur, Nqb, Nc, kmax;
+  int32_t has_box_full;   // 1: tensor maps with a full-block box exist (T_f >= block)
+  float scale_log2;       // softmax_scale * log2(e)
+  const int32_t *frame_idx;
+  const int32_t *sel_idx;
+  const int32_t *sel_cnt;
+  uint16_t *o;
+  float *lse;
+};
+
+// launches (defined in the .cu files); return cudaError_t as int
+int launch_select(const SelectParams &sp, const BatchMeta &meta, cudaStream_t st, int64_t *n_launches);
+int launch_attn(const AttnParams &ap, const BatchMeta &meta, int d, int blk, const CUtensorMap &tm_q,
+                const CUtensorMap &tm_k_full, const CUtensorMap &tm_k_8, const CUtensorMap &tm_v_full,
+                const CUtensorMap &tm_v_8, cudaStream_t st, int64_t *n_launches);
+
+}  // namespace li

@@ -1,0 +1,114 @@
+"""CPU-only checks of the boundary: libli.so builds for sm_100a, loads, exports every function include/li.h
+declares, and rejects bad arguments on the host before any CUDA call (no compute without a GPU)."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_2605_31158_b200 as li
+from paper_2605_31158_b200 import build as libuild
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def L():
+    libuild.build()
+    return li.lib()
+
+
+def declared_functions():
+    src = open(os.path.join(ROOT, "include", "li.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(li_[a-z_]+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported(L):
+    names = declared_functions()
+    assert set(names) == set(li.EXPORTS)
+    for n in names:
+        assert getattr(L, n) is not None
+    assert li.version() == 100
+    assert li.strerror(0) == "ok" and "unsupported" in li.strerror(li.LI_ERR_UNSUPPORTED)
+
+
+def test_sass_contains_tcgen05_and_tma():
+    """The attention kernel must be the Blackwell-native path: UTC*MMA (tcgen05.mma), LDTM/STTM, UTMALDG (TMA)."""
+    import shutil
+    import subprocess
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump):
+        pytest.skip("cuobjdump not available")
+    libuild.build()
+    sass = subprocess.run([cuobjdump, "-sass", li.LIB_PATH], capture_output=True, text=True).stdout
+    for mnemonic in ("UTCHMMA", "LDTM", "STTM", "UTMALDG"):
+        assert mnemonic in sass, mnemonic
+    assert "HMMA.16816" not in sass            # no legacy mma.sync path
+
+
+def make_problem(**over):
+    """A structurally valid li_problem with fake (aligned, never dereferenced) device addresses."""
+    fo = np.asarray([0, 4], dtype=np.int32)
+    p = li.li_problem()
+    p.B, p.H, p.Lq, p.d = 1, 2, 256, 64
+    p.frame_tokens, p.block_q, p.block_k, p.n_pages = 256, 64, 64, 8
+    p.q = 0x10000
+    p.q_sb, p.q_sh, p.q_st = 2 * 256 * 64, 256 * 64, 64
+    p.k_cache, p.v_cache = 0x20000, 0x30000
+    p.kv_sp, p.kv_sh, p.kv_st = 2 * 256 * 64, 256 * 64, 64
+    p.frame_idx = 0x40000
+    p.frame_off_host = fo.ctypes.data
+    p.n_cur_frames = 1
+    p.softmax_scale = 0.0
+    for k, v in over.items():
+        setattr(p, k, v)
+    return p, fo
+
+
+def test_workspace_bytes_and_validation(L):
+    p, fo = make_problem()
+    ws = L.li_workspace_bytes(ctypes.byref(p), 8)
+    # qbar [1,2,4,64] fp32 + kbar [1,2,12,64] fp32, each rounded up to 256 B
+    assert ws == 2 * 4 * 64 * 4 + 2 * 12 * 64 * 4
+    tk = np.asarray([8], dtype=np.int32)
+
+    def select(prob, kmax=8, ws_ptr=0x50000, ws_bytes=ws, sel=0x60000, cnt=0x70000):
+        return L.li_block_select(ctypes.byref(prob), tk.ctypes.data, kmax, sel, cnt, None, 0, ws_ptr, ws_bytes, None)
+
+    def attn(prob, o=0x80000):
+        return L.li_sparse_attn(ctypes.byref(prob), 0x60000, 0x70000, 8, o, None, None, 0, None)
+
+    for bad, code in ((dict(d=96), li.LI_ERR_UNSUPPORTED), (dict(block_q=128), li.LI_ERR_UNSUPPORTED),
+                      (dict(block_q=32, block_k=32), li.LI_ERR_UNSUPPORTED), (dict(B=65), li.LI_ERR_UNSUPPORTED),
+                      (dict(frame_tokens=250), li.LI_ERR_INVALID_ARG), (dict(q=0), li.LI_ERR_INVALID_ARG),
+                      (dict(q=0x10008), li.LI_ERR_INVALID_ARG), (dict(kv_st=60), li.LI_ERR_INVALID_ARG),
+                      (dict(Lq=100), li.LI_ERR_INVALID_ARG), (dict(n_cur_frames=5), li.LI_ERR_INVALID_ARG),
+                      (dict(softmax_scale=-1.0), li.LI_ERR_INVALID_ARG), (dict(H=0), li.LI_ERR_INVALID_ARG)):
+        pb, keep = make_problem(**bad)
+        assert select(pb) == code, bad
+        assert attn(pb) == code, bad
+        assert L.li_workspace_bytes(ctypes.byref(pb), 8) == 0
+    assert select(p, kmax=4) == li.LI_ERR_INVALID_ARG           # kmax < k_b
+    assert select(p, ws_bytes=ws - 1) == li.LI_ERR_WORKSPACE
+    assert select(p, ws_ptr=0) == li.LI_ERR_WORKSPACE
+    assert select(p, ws_ptr=0x50010) == li.LI_ERR_WORKSPACE     # not 256-byte aligned
+    assert select(p, sel=0) == li.LI_ERR_INVALID_ARG
+    assert attn(p, o=0) == li.LI_ERR_INVALID_ARG
+    assert L.li_block_select(None, tk.ctypes.data, 8, 1, 1, None, 0, 1, 1, None) == li.LI_ERR_INVALID_ARG
+
+
+def test_binding_refuses_cpu_tensors():
+    import torch
+    q = torch.zeros((1, 2, 256, 64), dtype=torch.bfloat16)
+    kc = torch.zeros((8, 2, 256, 64), dtype=torch.bfloat16)
+    with pytest.raises(ValueError):
+        li.Context(q, kc, kc, torch.zeros(4, dtype=torch.int32), [0, 4], 1, 64)
+
+
+def test_missing_library_fails_loudly(monkeypatch, tmp_path):
+    monkeypatch.setattr(li, "_lib", None)
+    monkeypatch.setattr(li, "LIB_PATH", str(tmp_path / "nope.so"))
+    with pytest.raises(RuntimeError, match="no CPU fallback"):
+        li.lib()

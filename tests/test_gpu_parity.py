@@ -1,0 +1,154 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C-ABI binding, against oracle/li_oracle.py on the
+same seeded inputs.  Bars (BASELINE.json north_star): block mask bit-exact except reported ties within 1e-4
+relative of the k-th score; attention output max-abs <= 2e-2 and mean-abs <= 2e-3 against the oracle."""
+from fractions import Fraction
+
+import numpy as np
+import pytest
+import torch
+
+import li_workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def P():
+    from tests import parity_util
+    return parity_util
+
+
+def test_tiny_config_full_parity(P):
+    """BASELINE.json configs[0]: B=1,H=2,d=64,T_f=256,Lq=256, frames {0,3}|{6}|{7}, block 64, top-k 8."""
+    prob = W.build(W.spec_tiny())
+    assert prob.M(0) == 12 and prob.Nqb == 4 and int(prob.top_k[0]) == 8
+    excused, mx, mean = P.full_parity(prob)
+    print(f"tiny: excused={excused} max-abs={mx:.3g} mean-abs={mean:.3g}")
+
+
+@pytest.mark.parametrize("d,block,T_f", [(128, 128, 200), (64, 128, 200), (128, 64, 72), (64, 64, 40), (128, 128, 1560)])
+def test_small_full_parity_straddling_blocks(P, d, block, T_f):
+    """Reduced shapes: T_f not a multiple of the block (blocks straddle frames, 8-row TMA pieces), ragged
+    history and chunk tails, unsorted memory pages, several query tiles."""
+    n_cur = 1 if T_f == 1560 else 3
+    spec = W.spec_small(name=f"small-d{d}-b{block}-t{T_f}", H=2, d=d, block=block, frame_tokens=T_f,
+                        n_cur_frames=n_cur, n_pages=12, n_mem=(2,), n_win=(3,) if T_f != 1560 else (1,),
+                        density=Fraction(1, 2))
+    prob = W.build(spec)
+    excused, mx, mean = P.full_parity(prob)
+    print(f"{spec.name}: M={prob.M(0)} k={int(prob.top_k[0])} excused={excused} max-abs={mx:.3g} mean-abs={mean:.3g}")
+
+
+def test_small_varlen_batch_and_no_memory_calls(P):
+    """adaptive-like: several independent calls in one launch, ragged Lk, calls without retrieved memory."""
+    spec = W.spec_small(name="small-adaptive", H=2, d=128, block=128, frame_tokens=200, n_cur_frames=2,
+                        n_pages=40, n_mem=(0, 2, 0, 3), n_win=(1, 2, 4, 1), density=Fraction(3, 10),
+                        pages_per_call=10)
+    prob = W.build(spec)
+    assert prob.B == 4 and len(set(prob.M(b) for b in range(4))) > 1
+    excused, mx, mean = P.full_parity(prob)
+    print(f"small-adaptive: excused={excused} max-abs={mx:.3g} mean-abs={mean:.3g}")
+
+
+def test_dense_equivalence_small(P):
+    """r = 1: every block selected -> equals dense attention over the whole gathered context (torch SDPA on CPU,
+    fp32, as an independent library routine) and the oracle."""
+    spec = W.spec_small(name="small-dense", H=2, d=128, block=128, frame_tokens=200, n_cur_frames=2,
+                        n_pages=10, n_mem=(2,), n_win=(2,), density=Fraction(1, 1))
+    prob = W.build(spec)
+    ctx, buf = P.run_gpu(prob)
+    M = prob.M(0)
+    sel = buf.sel_idx.cpu().numpy()[0]
+    assert (sel == np.arange(M)).all()
+    frames = prob.frame_idx
+    K = torch.cat([prob.k_cache[int(p)] for p in frames], dim=1).float()     # [H, Lk, d]
+    V = torch.cat([prob.v_cache[int(p)] for p in frames], dim=1).float()
+    ref = torch.nn.functional.scaled_dot_product_attention(prob.q[0].float(), K, V)
+    diff = (buf.o[0].float().cpu() - ref).abs()
+    assert diff.max() <= P.MAX_ABS and diff.mean() <= P.MEAN_ABS
+
+
+def test_degenerate_topk_zero_and_no_history(P):
+    """k = 0 -> chunk-only attention; a call with no history frames at all (M = 0)."""
+    spec = W.spec_small(name="small-k0", H=2, d=128, block=128, frame_tokens=200, n_cur_frames=2, n_pages=10,
+                        n_mem=(1, 0), n_win=(2, 0), top_k=0, pages_per_call=5)
+    prob = W.build(spec)
+    assert prob.M(1) == 0
+    ctx, buf = P.run_gpu(prob)
+    assert (buf.sel_cnt == 0).all() and (buf.sel_idx == -1).all()
+    o_ref, lse_ref = P.oracle_attn(prob, [np.zeros((2, prob.Nqb, 0), np.int32)] * 2)
+    P.compare_output(buf.o, buf.lse, o_ref, lse_ref)
+
+
+def test_no_chunk_history_only_and_softmax_scale(P):
+    """n_cur_frames = 0 (the API's 'other reading' of density): queries attend selected history only."""
+    import paper_2605_31158_b200 as li
+    from oracle import li_oracle as O
+    g = torch.Generator().manual_seed(99)
+    H, d, T_f, blk, Lq = 2, 128, 200, 128, 300
+    q = torch.randn((1, H, Lq, d), generator=g).to(torch.bfloat16)
+    kc = torch.randn((5, H, T_f, d), generator=g).to(torch.bfloat16)
+    vc = torch.randn((5, H, T_f, d), generator=g).to(torch.bfloat16)
+    fi = np.asarray([3, 1, 4], np.int32)
+    fo = np.asarray([0, 3], np.int32)
+    ctx = li.Context(q.cuda(), kc.cuda(), vc.cuda(), torch.from_numpy(fi).cuda(), fo, 0, blk, softmax_scale=0.05)
+    buf = li.Buffers(ctx, 3, want_scores=True)
+    li.forward(ctx, [3], buf)
+    torch.cuda.synchronize()
+    u16 = lambda t: t.view(torch.int16).numpy().view(np.uint16)
+    osel, osc = O.block_select(u16(q), u16(kc), fi, fo, 0, blk, blk, [3])
+    np.testing.assert_array_equal(buf.sel_idx.cpu().numpy()[0], osel[0])
+    o_ref, lse_ref = O.sparse_attn(u16(q), u16(kc), u16(vc), fi, fo, 0, blk, blk, osel, softmax_scale=0.05)
+    P.compare_output(buf.o, buf.lse, o_ref, lse_ref)
+
+
+def test_exact_ties_lowest_index_and_page_permutation(P):
+    """Duplicate page ids -> bit-identical pooled blocks -> exact ties: the GPU must pick the lowest index.
+    Permuting the pool and rewriting the list must give bit-identical GPU results (gather correctness)."""
+    import paper_2605_31158_b200 as li
+    g = torch.Generator().manual_seed(5)
+    H, d, T_f, blk = 2, 64, 64, 64
+    q = torch.randn((1, H, T_f, d), generator=g).to(torch.bfloat16)
+    kc = torch.randn((4, H, T_f, d), generator=g).to(torch.bfloat16)
+    vc = torch.randn((4, H, T_f, d), generator=g).to(torch.bfloat16)
+    fi = np.asarray([1, 0, 1, 0, 1, 2], np.int32)
+    fo = np.asarray([0, 6], np.int32)
+
+    def run(kc_, vc_, fi_, k):
+        ctx = li.Context(q.cuda(), kc_.cuda(), vc_.cuda(), torch.from_numpy(fi_).cuda(), fo, 1, blk)
+        buf = li.Buffers(ctx, 5, want_scores=True)
+        li.forward(ctx, [k], buf)
+        torch.cuda.synchronize()
+        return buf
+
+    b1 = run(kc, vc, fi, 1)
+    sc = b1.scores.cpu().numpy()[0, :, 0]
+    for h in range(H):
+        assert sc[h, 0] == sc[h, 2] == sc[h, 4] and sc[h, 1] == sc[h, 3]
+        assert int(b1.sel_idx[0, h, 0, 0]) == (0 if sc[h, 0] >= sc[h, 1] else 1)
+    b2 = run(kc, vc, fi, 2)
+    for h in range(H):
+        assert b2.sel_idx[0, h, 0, :2].tolist() == ([0, 2] if sc[h, 0] >= sc[h, 1] else [1, 3])
+    perm = torch.tensor([2, 0, 3, 1])
+    inv = torch.argsort(perm).numpy()
+    b3 = run(kc[perm], vc[perm], inv[fi].astype(np.int32), 2)
+    assert torch.equal(b2.sel_idx, b3.sel_idx) and torch.equal(b2.o, b3.o) and torch.equal(b2.scores, b3.scores)
+
+
+def test_constant_v_and_nan_in_unused_pages(P):
+    """V constant -> O equals it for any mask; pages not on the frame list are NaN and must never be touched."""
+    import paper_2605_31158_b200 as li
+    spec = W.spec_small(name="small-nan", H=2, d=128, block=128, frame_tokens=200, n_cur_frames=2, n_pages=12,
+                        n_mem=(2,), n_win=(2,), density=Fraction(1, 2))
+    prob = W.build(spec)
+    used = set(int(p) for p in prob.frame_idx)
+    for pg in range(spec.n_pages):
+        if pg not in used:
+            prob.k_cache[pg] = float("nan")
+            prob.v_cache[pg] = float("nan")
+    for pg in used:
+        prob.v_cache[pg] = 0.75
+    ctx, buf = P.run_gpu(prob)
+    o = buf.o.float().cpu()
+    assert torch.isfinite(o).all() and (o - 0.75).abs().max() < 1e-2
+    assert torch.isfinite(buf.scores.cpu()[..., :prob.M(0)]).all()
