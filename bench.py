@@ -1,0 +1,334 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the Light Interaction sparse-attention hot path on B200.
+
+A "step" = one pass of the whole hot path (li_block_select + li_sparse_attn) over
+one synthetic `mid` workload (BASELINE.json configs[1]; the config `metric` is quoted on).  value = effective
+TFLOP/s counted over attended blocks only (4*d*valid_q*valid_k per (head, query block), from the actual mask).
+Multi-GPU: the path has no exchange step: `--gpus N` runs N independent replicas, one per
+rank, weak scaling, no collective on the data path.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config mid|long|tiny|adaptive|dense-equivalence]
+  python bench.py --impl reference ...      # times the CPU oracle (oracle/li_oracle.py) on a bounded sample
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+import torch
+
+import li_workloads as W
+
+METRIC = "sparse-attn effective TFLOP/s over attended blocks (select + attention, ms/call in ms_per_step)"
+UNIT = "TFLOP/s"
+# dram__bytes_read.sum + dram__bytes_write.sum of li_sparse_attn_kernel<128,128> per launch, from the
+# `ncu --set full` capture summarised in profiles/ (None until that capture exists for this workload).
+NCU_TRAFFIC_BYTES = {"mid": None}
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return {"bf16_tflops": float(d["bf16_tflops"]), "bf16_tflops_sustained": float(d.get("bf16_tflops_sustained", d["bf16_tflops"])),
+                "hbm_gbs": float(d["hbm_gbs"]), "source": "measured"}
+    return {"bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "hbm_gbs": 6650.0, "source": "fallback"}
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.stop = index, [], threading.Event()
+        self.t = threading.Thread(target=self._run, daemon=True)
+
+    def _run(self):
+        while not self.stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i", str(self.index)],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([x.strip() for x in out.split(",")])
+            except Exception:
+                pass
+            self.stop.wait(0.1)
+
+    def __enter__(self):
+        self.t.start()
+        return self
+
+    def __exit__(self, *a):
+        self.stop.set()
+        self.t.join(timeout=6)
+
+    def summary(self):
+        sm, mx, reasons = [], 0.0, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = max(mx, float(r[1]))
+                for n, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                continue
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx or None, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------ CPU oracle arm
+def oracle_sample(prob: W.Problem, n_heads: int, tiles_per_head=None):
+    """Times oracle/li_oracle.py, as it stands, on a bounded sample of `prob`: the first n_heads heads of call 0
+    (select for those heads + attention for their query blocks).  Returns (seconds, effective flops, description)."""
+    from oracle import li_oracle as O
+    s = prob.spec
+    nh = min(n_heads, s.H)
+    q = prob.u16(prob.q[:1, :nh].contiguous())
+    kc = prob.u16(prob.k_cache[:, :nh].contiguous())
+    vc = prob.u16(prob.v_cache[:, :nh].contiguous())
+    fi = prob.frame_idx[prob.frame_off[0]:prob.frame_off[1]]
+    fo = np.asarray([0, len(fi)], np.int32)
+    tiles = None
+    nq = prob.Nqb if tiles_per_head is None else min(tiles_per_head, prob.Nqb)
+    if tiles_per_head is not None:
+        tiles = [(0, h, i) for h in range(nh) for i in range(nq)]
+    t0 = time.perf_counter()
+    sel, _ = O.block_select(q, kc, fi, fo, s.n_cur_frames, s.block, s.block, prob.top_k[:1])
+    O.sparse_attn(q, kc, vc, fi, fo, s.n_cur_frames, s.block, s.block, sel, tiles=tiles)
+    dt = time.perf_counter() - t0
+    sub = W.Problem(s, prob.q[:1, :nh], prob.k_cache, prob.v_cache, fi, fo, prob.top_k[:1])
+    cnt = np.full((nh, prob.Nqb), sel[0].shape[-1], np.int32)
+    flops = 0
+    Lc = s.n_cur_frames * s.frame_tokens
+    Lh, M = sub.L_hist(0), sub.M(0)
+    tail = Lh - (M - 1) * s.block if M > 0 else 0
+    for h in range(nh):
+        for i in range(nq):
+            vq = min(s.block, sub.Lq - i * s.block)
+            kv = Lc + sum((tail if int(m) == M - 1 else s.block) for m in sel[0][h, i])
+            flops += 4 * s.d * vq * kv
+    desc = f"{s.name}: call 0, heads 0..{nh - 1} of {s.H}, query blocks 0..{nq - 1} of {prob.Nqb}, select + attention"
+    return dt, flops, desc
+
+
+def cpu_threads() -> int:
+    try:
+        from threadpoolctl import threadpool_info
+        n = [int(i.get("num_threads", 1)) for i in threadpool_info() if i.get("user_api") == "blas"]
+        if n:
+            return max(n)
+    except Exception:
+        pass
+    return os.cpu_count() or 1
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    prob = W.build(W.spec_by_name(args.config, H=args.ref_heads if args.config != "tiny" else None))
+    times, flops, desc = [], 0, ""
+    for it in range(args.warmup + args.steps):
+        dt, flops, desc = oracle_sample(prob, args.ref_heads, args.ref_tiles)
+        if it >= args.warmup:
+            times.append(dt)
+    t = float(np.mean(times))
+    val = flops / t / 1e12
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.config, "sample": desc},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cpu_threads(), "kind": "oracle", "sample": desc},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------ CUDA arm
+def run_cuda(args):
+    import torch.distributed as dist
+
+    import paper_2605_31158_b200 as li
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    li.lib()                                   # fail loudly if libli.so is missing
+
+    spec = W.spec_by_name(args.config)
+    prob = W.build(spec)                       # every rank: an independent replica of the same workload
+    s = prob.spec
+    # host side (pinned): what changes every step in the AR loop = Q, the chunk's K/V pages, the frame list
+    q_host = prob.q.pin_memory()
+    fi_host = torch.from_numpy(prob.frame_idx).pin_memory()
+    cur_pages = sorted(set(int(prob.frame_idx[prob.frame_off[b + 1] - 1 - j]) for b in range(prob.B)
+                           for j in range(s.n_cur_frames)))
+    kcur_host = prob.k_cache[cur_pages].pin_memory()
+    vcur_host = prob.v_cache[cur_pages].pin_memory()
+    cur_idx = torch.tensor(cur_pages, device=dev)
+
+    q = prob.q.to(dev)
+    kc = prob.k_cache.to(dev)
+    vc = prob.v_cache.to(dev)
+    fi = torch.from_numpy(prob.frame_idx).to(dev)
+    ctx = li.Context(q, kc, vc, fi, prob.frame_off, s.n_cur_frames, s.block)
+    buf = li.Buffers(ctx, prob.kmax, want_scores=False, want_lse=True)
+    o_host = torch.empty(buf.o.shape, dtype=buf.o.dtype).pin_memory()
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)   # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def step(ev=None):
+        if ev is not None:
+            ev[0].record(stream)
+        li.li_block_select(ctx, prob.top_k, buf.kmax, buf.sel_idx, buf.sel_cnt, buf.workspace, None, stream)
+        if ev is not None:
+            ev[1].record(stream)
+        li.li_sparse_attn(ctx, buf.sel_idx, buf.sel_cnt, buf.kmax, buf.o, buf.lse, buf.workspace, stream)
+        if ev is not None:
+            ev[2].record(stream)
+
+    def e2e_step():
+        q.copy_(q_host, non_blocking=True)
+        fi.copy_(fi_host, non_blocking=True)
+        if contiguous_cur:
+            kc[cur_pages[0]:cur_pages[-1] + 1].copy_(kcur_host, non_blocking=True)
+            vc[cur_pages[0]:cur_pages[-1] + 1].copy_(vcur_host, non_blocking=True)
+        else:
+            kc.index_copy_(0, cur_idx, kcur_host.to(dev, non_blocking=True))
+            vc.index_copy_(0, cur_idx, vcur_host.to(dev, non_blocking=True))
+        step()
+        o_host.copy_(buf.o, non_blocking=True)
+
+    contiguous_cur = cur_pages == list(range(cur_pages[0], cur_pages[-1] + 1))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(3, args.warmup)):
+        flush.fill_(1)
+        step()
+    torch.cuda.synchronize()
+    sel_idx = buf.sel_idx.cpu().numpy()
+    sel_cnt = buf.sel_cnt.cpu().numpy()
+    flops = W.effective_flops(prob, [sel_idx[b] for b in range(prob.B)], [sel_cnt[b] for b in range(prob.B)])
+
+    # ---- device-resident timing: K steps, L2 flushed between them, CUDA events on the launching stream ----
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    li.reset_launch_count()
+    barrier()
+    with ClockSampler(local) as clk:
+        t_wall0 = time.perf_counter()
+        for k in range(args.steps):
+            flush.fill_(k & 0xff)
+            step(evs[k])
+        barrier()
+        launches = li.launch_count()            # counted by the library inside the timed region
+        t_wall = time.perf_counter() - t_wall0
+        while time.perf_counter() - t_wall0 < 0.6:      # very short runs: keep the same load up until the
+            step()                                      # sampler has a few readings (not timed, not counted)
+            torch.cuda.synchronize()
+    sel_ms = np.asarray([e[0].elapsed_time(e[1]) for e in evs])
+    att_ms = np.asarray([e[1].elapsed_time(e[2]) for e in evs])
+    step_ms = np.asarray([e[0].elapsed_time(e[2]) for e in evs])
+    total_ms = float(step_ms.sum())
+
+    # ---- end to end: pinned host -> device copies of the step's inputs and device -> host read of O, timed ----
+    for _ in range(2):
+        e2e_step()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for k in range(args.steps):
+        e2e_step()
+    e1.record(stream)
+    barrier()
+    e2e_ms = e0.elapsed_time(e1)
+    h2d = q_host.numel() * 2 + fi_host.numel() * 4 + kcur_host.numel() * 2 + vcur_host.numel() * 2
+    d2h = o_host.numel() * 2
+
+    t = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms, e2e_ms = float(t[0]), float(t[1])
+    if rank == 0:
+        pk = peaks()
+        value = world * flops * args.steps / (total_ms * 1e-3) / 1e12
+        e2e_val = world * flops * args.steps / (e2e_ms * 1e-3) / 1e12
+        attn_tflops = flops / (float(att_ms.mean()) * 1e-3) / 1e12
+        sel_bytes = sum((prob.Lq + prob.L_hist(b)) * s.d * 2 * s.H for b in range(prob.B))
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
+            "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "bf16", "data": "synthetic",
+            "config": {"workload": s.name, "B": prob.B, "H": s.H, "d": s.d, "Lq": prob.Lq, "frame_tokens": s.frame_tokens,
+                       "block": s.block, "Lk": [prob.L_hist(b) + prob.Lq for b in range(prob.B)],
+                       "top_k": [int(x) for x in prob.top_k], "M": [prob.M(b) for b in range(prob.B)],
+                       "l2": "flushed between timed steps (256 MiB write)", "multi_gpu": "replicas only (no collective)"},
+            "effective_flops_per_step": int(flops),
+            "select_ms": float(sel_ms.mean()), "attn_ms": float(att_ms.mean()), "attn_ms_min": float(att_ms.min()),
+            "select_overhead_frac_of_attn": float(sel_ms.mean() / att_ms.mean()),
+            "select_gbs": sel_bytes / (float(sel_ms.mean()) * 1e-3) / 1e9,
+            "frac_of_peak_burst": attn_tflops / pk["bf16_tflops"], "frac_of_peak_sustained": attn_tflops / pk["bf16_tflops_sustained"],
+            "roofline": {"bound": "tensor", "achieved": attn_tflops, "peak": pk["bf16_tflops"], "unit": "TFLOP/s",
+                         "frac": attn_tflops / pk["bf16_tflops"], "traffic": NCU_TRAFFIC_BYTES.get(s.name),
+                         "kernel": "li_sparse_attn_kernel", "peak_source": pk["source"] + " burst bf16"},
+            "roofline_select": {"bound": "hbm", "achieved": sel_bytes / (float(sel_ms.mean()) * 1e-3) / 1e9, "peak": pk["hbm_gbs"],
+                                "unit": "GB/s", "frac": sel_bytes / (float(sel_ms.mean()) * 1e-3) / 1e9 / pk["hbm_gbs"],
+                                "kernel": "li_pool_kernel + li_score_topk_kernel"},
+            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                    "ms_per_step": e2e_ms / args.steps,
+                    "note": "per step: Q, frame list and the chunk's K/V pages copied from pinned host memory, O read back; "
+                            "the historical K/V cache stays resident (it is the cache)"},
+            "gpu_launches": int(launches), "clocks": clk.summary(),
+        }
+        if not args.no_cpu and world == 1:
+            dt, fl, desc = oracle_sample(prob, args.ref_heads, args.ref_tiles)
+            line["cpu_baseline"] = {"value": fl / dt / 1e12, "unit": UNIT, "cores": cpu_threads(), "kind": "oracle",
+                                    "sample": desc, "seconds": dt}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--config", default="mid", choices=["tiny", "mid", "long", "adaptive", "dense-equivalence"])
+    ap.add_argument("--ref-heads", type=int, default=2, help="heads in the oracle's bounded sample")
+    ap.add_argument("--ref-tiles", type=int, default=None, help="query blocks per head in the oracle's sample (default all)")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        if args.steps == 20 and args.warmup == 5:
+            args.steps, args.warmup = 2, 1
+        return run_reference(args)
+    return run_cuda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
