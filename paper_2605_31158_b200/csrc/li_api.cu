@@ -153,15 +153,16 @@ int li_sparse_attn(const li_problem *p, const int32_t *sel_idx, const int32_t *s
   if ((uintptr_t)o & 15u) return LI_ERR_INVALID_ARG;
 
   const int blk = p->block_k;
-  const int has_full = p->frame_tokens >= blk ? 1 : 0;
+  const int half = blk / 2;                 // K/V are fetched as half-tiles of blk/2 rows
+  const int has_full = p->frame_tokens >= half ? 1 : 0;
   CUtensorMap tm_q, tm_kf, tm_k8, tm_vf, tm_v8;
   bool ok = encode_map(&tm_q, p->q, p->d, p->Lq, p->H, p->B, p->q_st, p->q_sh, p->q_sb, blk);
   ok = ok && encode_map(&tm_k8, p->k_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp, 8);
   ok = ok && encode_map(&tm_v8, p->v_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp, 8);
   ok = ok && encode_map(&tm_kf, p->k_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp,
-                        has_full ? blk : 8);
+                        has_full ? half : 8);
   ok = ok && encode_map(&tm_vf, p->v_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp,
-                        has_full ? blk : 8);
+                        has_full ? half : 8);
   if (!ok) return LI_ERR_CUDA;
 
   li::AttnParams ap;

@@ -2,13 +2,17 @@
 // (Eq. 11), K/V tiles fetched IN PLACE from the frame-paged cache by TMA with the page
 // as a tensor coordinate (replaces the paper's KV-Prep / Untile-Scatter copies).
 //
-// One CTA = one query block (BLK query rows, padded to the 128-row UMMA tile) of one (call, head).
-// Two CTAs are resident per SM (256 TMEM columns and ~98 KB of shared memory each), so that one CTA's
-// softmax overlaps the other CTA's MMAs.
-//   warps 0-3 : softmax + correction + epilogue; warp w owns TMEM lanes 32w..32w+31 (one query row per thread)
-//   warp 4    : TMA producer (one elected lane): Q once, then K_j / V_j per attended block
+// One CTA = one query block (BLK query rows, padded to the 128-row UMMA tile) of one (call, head); two CTAs per SM.
+// Every attended KV block is processed as two HALF-tiles of HALF = BLK/2 keys, software-pipelined inside the CTA:
+// S is double-buffered in TMEM, so the tensor core computes S(t+1) = Q K(t+1)^T while the softmax warps work on
+// S(t), and O += P(t) V(t) is issued as soon as P(t) is written.  Tensor-core issue order:
+//     QK(0) QK(1) | PV(0) QK(2) | PV(1) QK(3) | ...      (K/V half-tiles are loaded in exactly this order
+//                                                         into a 4-slot shared-memory ring)
+//   warps 0-3 : softmax + lazy correction + epilogue; warp w owns TMEM lanes 32w..32w+31 (one query row per thread)
+//   warp 4    : TMA producer (one elected lane): Q once, then the K/V half-tiles
 //   warp 5    : TMEM allocation and the single-thread tcgen05.mma issuer
-// TMEM: columns [0,BLK) S (fp32), overlaid by P (bf16, BLK/2 columns) once S has been read; [128,128+D) O.
+// TMEM (256 columns): [0,HALF) S_a, [64,64+HALF) S_b (fp32; P in bf16 overlays the first HALF/2 columns of its S
+// buffer once S has been read), [128,128+D) O.
 #include "li_internal.h"
 #include "li_ptx.cuh"
 
@@ -16,24 +20,35 @@ namespace li {
 
 constexpr int kSelCap = 1024;       // selected-block indices staged in shared memory (rest read from global)
 constexpr int kTmemCols = 256;
+constexpr int kSbCol = 64;
 constexpr int kOCol = 128;
+constexpr int kStages = 4;
 constexpr float kRescaleThreshold = 8.0f;   // log2 units: P stays <= 2^8 between lazy rescales
 
 template <int D, int BLK>
 struct AttnSmem {
+  static constexpr int HALF = BLK / 2;
   static constexpr int kQChunk = 128 * 128;            // bytes of one 64-column chunk of the 128-row Q tile
-  static constexpr int kKVChunk = BLK * 128;           // bytes of one 64-column chunk of a K or V tile
+  static constexpr int kKVChunk = HALF * 128;          // bytes of one 64-column chunk of a K or V half-tile
   static constexpr int kQ = (D / 64) * kQChunk;
-  static constexpr int kKV = (D / 64) * kKVChunk;
+  static constexpr int kStage = (D / 64) * kKVChunk;
   static constexpr int kOffQ = 0;
-  static constexpr int kOffK = kQ;
-  static constexpr int kOffV = kQ + kKV;
-  static constexpr int kOffSel = kQ + 2 * kKV;
+  static constexpr int kOffRing = kQ;
+  static constexpr int kOffSel = kQ + kStages * kStage;
   static constexpr int kOffBar = kOffSel + kSelCap * 4;
-  static constexpr int kTotal = kOffBar + 128 + 1024;  // + barriers + slack for 1024-B alignment
+  static constexpr int kTotal = kOffBar + 256 + 1024;  // + barriers + slack for 1024-B alignment
 };
 
-enum { BAR_Q_FULL = 0, BAR_K_FULL, BAR_K_EMPTY, BAR_V_FULL, BAR_V_EMPTY, BAR_S_FULL, BAR_P_FULL, BAR_O_FULL, BAR_COUNT };
+enum {
+  BAR_Q_FULL = 0,
+  BAR_FULL = 1,                    // +slot
+  BAR_EMPTY = BAR_FULL + kStages,  // +slot
+  BAR_S_FULL = BAR_EMPTY + kStages,  // +buffer
+  BAR_P_FULL = BAR_S_FULL + 2,       // +buffer
+  BAR_PV_DONE = BAR_P_FULL + 2,
+  BAR_O_FULL,
+  BAR_COUNT
+};
 
 template <int D, int BLK>
 __global__ void __launch_bounds__(192, 2)
@@ -41,10 +56,11 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
                       const __grid_constant__ CUtensorMap tm_k_full, const __grid_constant__ CUtensorMap tm_k_8,
                       const __grid_constant__ CUtensorMap tm_v_full, const __grid_constant__ CUtensorMap tm_v_8) {
   using L = AttnSmem<D, BLK>;
+  constexpr int HALF = L::HALF;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   uint8_t *smem = smem_raw + (smem_base - smem_u32(smem_raw));
-  const uint32_t sQ = smem_base + L::kOffQ, sK = smem_base + L::kOffK, sV = smem_base + L::kOffV;
+  const uint32_t sQ = smem_base + L::kOffQ, sRing = smem_base + L::kOffRing;
   int32_t *sSel = reinterpret_cast<int32_t *>(smem + L::kOffSel);
   const uint32_t bar0 = smem_base + L::kOffBar;
   uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + L::kOffBar + 8 * BAR_COUNT);
@@ -66,6 +82,7 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
   const int32_t *sel_row = p.sel_idx + row_id * p.kmax;
   const int n_tiles = Nc + cnt;
   const int valid_q = min(BLK, p.Lq - i * BLK);
+  const int tail_cur = L_cur - (Nc - 1) * BLK, tail_hist = L_hist - (M - 1) * BLK;
 
   // ---- one-time setup ----
   for (int t = threadIdx.x; t < cnt && t < kSelCap; t += blockDim.x) sSel[t] = sel_row[t];
@@ -75,7 +92,7 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
     tma_prefetch_desc(&tm_v_full);
     tma_prefetch_desc(&tm_k_8);
     tma_prefetch_desc(&tm_v_8);
-    for (int k = 0; k < BAR_COUNT; ++k) mbar_init(bar(k), k == BAR_P_FULL ? 4 : 1);
+    for (int k = 0; k < BAR_COUNT; ++k) mbar_init(bar(k), (k == BAR_P_FULL || k == BAR_P_FULL + 1) ? 4 : 1);
     mbar_fence_init();
     fence_proxy_async();
   }
@@ -89,8 +106,17 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
   const uint32_t tmem = *tmem_slot;
 
   auto sel_at = [&](int jj) -> int { return jj < kSelCap ? sSel[jj] : sel_row[jj]; };
+  // valid key columns of attended tile j (chunk blocks first, then the selected historical blocks)
+  auto tile_valid = [&](int j) -> int {
+    if (j < Nc) return j == Nc - 1 ? tail_cur : BLK;
+    return sel_at(j - Nc) == M - 1 ? tail_hist : BLK;
+  };
+  // number of half-tiles with at least one valid key (a half-tile without any is skipped by every role)
+  int T = 2 * n_tiles;
+  if (Nc > 0 && tail_cur <= HALF) --T;
+  if (cnt > 0 && sel_at(cnt - 1) == M - 1 && tail_hist <= HALF) --T;
 
-  if (n_tiles > 0) {
+  if (T > 0) {
     if (warp == 4) {
       // =============================== TMA producer ===============================
       if (lane == 0) {
@@ -98,21 +124,31 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
 #pragma unroll
         for (int c = 0; c < D / 64; ++c) tma_load_4d(sQ + c * L::kQChunk, &tm_q, bar(BAR_Q_FULL), c * 64, i * BLK, h, b);
 
-        auto issue_tile = [&](const CUtensorMap *tm_full, const CUtensorMap *tm_8, uint32_t dst, uint32_t mb,
-                              const int32_t *pages, int t0, int region_len) {
-          const int t_last = min(t0 + BLK, region_len) - 1;
+        int n = 0;                                   // running load index: slot = n % 4
+        // loads HALF rows [t0, t0+HALF) of a region (history or chunk) into ring slot n % 4
+        auto load_half = [&](const CUtensorMap *tm_full, const CUtensorMap *tm_8, int j, int hh) {
+          const bool is_cur = j < Nc;
+          const int blk = is_cur ? j : sel_at(j - Nc);
+          const int32_t *pages = p.frame_idx + foff + (is_cur ? n_hist : 0);
+          const int region_len = is_cur ? L_cur : L_hist;
+          const int t0 = blk * BLK + hh * HALF;
+          const int slot = n & (kStages - 1);
+          const uint32_t dst = sRing + slot * L::kStage, mb = bar(BAR_FULL + slot);
+          mbar_wait(bar(BAR_EMPTY + slot), ((n >> 2) & 1) ^ 1);
+          mbar_arrive_expect_tx(mb, HALF * D * 2);
+          const int t_last = min(t0 + HALF, region_len) - 1;
           const int pg0 = t0 / p.T_f;
           if (p.has_box_full && pg0 == t_last / p.T_f) {
-            // whole block inside one page: one box per 64-column chunk; rows past the page end are
-            // zero-filled by the hardware (the region always ends on a page boundary)
+            // inside one page: one box per 64-column chunk; rows past the page end are zero-filled by the
+            // hardware (a region always ends on a page boundary)
             const int page = pages[pg0];
             const int row = t0 - pg0 * p.T_f;
 #pragma unroll
             for (int c = 0; c < D / 64; ++c) tma_load_4d(dst + c * L::kKVChunk, tm_full, mb, c * 64, row, h, page);
           } else {
-            // block straddles frames: 8-row pieces (one SWIZZLE_128B atom each, destinations stay 1024-B aligned)
+            // straddles frames: 8-row pieces (one SWIZZLE_128B atom each, destinations stay 1024-B aligned)
             int cur_pg = -1, page = 0;
-            for (int g = 0; g < BLK / 8; ++g) {
+            for (int g = 0; g < HALF / 8; ++g) {
               const int t = t0 + g * 8;
               int row = p.T_f;             // out of bounds -> zeros
               if (t < region_len) {
@@ -125,87 +161,108 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
                 tma_load_4d(dst + c * L::kKVChunk + g * 1024, tm_8, mb, c * 64, row, h, page);
             }
           }
+          ++n;
+        };
+        auto advance = [&](int &j, int &hh) {
+          if (hh == 0 && tile_valid(j) > HALF) hh = 1;
+          else { ++j; hh = 0; }
         };
 
-        for (int j = 0; j < n_tiles; ++j) {
-          const bool is_cur = j < Nc;
-          const int blk = is_cur ? j : sel_at(j - Nc);
-          const int32_t *pages = p.frame_idx + foff + (is_cur ? n_hist : 0);
-          const int region_len = is_cur ? L_cur : L_hist;
-          const uint32_t ph = (j & 1) ^ 1;
-          mbar_wait(bar(BAR_K_EMPTY), ph);
-          mbar_arrive_expect_tx(bar(BAR_K_FULL), BLK * D * 2);
-          issue_tile(&tm_k_full, &tm_k_8, sK, bar(BAR_K_FULL), pages, blk * BLK, region_len);
-          mbar_wait(bar(BAR_V_EMPTY), ph);
-          mbar_arrive_expect_tx(bar(BAR_V_FULL), BLK * D * 2);
-          issue_tile(&tm_v_full, &tm_v_8, sV, bar(BAR_V_FULL), pages, blk * BLK, region_len);
+        // load order == consumption order of the MMA warp: K0 K1 | V0 K2 | V1 K3 | ...
+        int kj = 0, kh = 0, vj = 0, vh = 0;
+        load_half(&tm_k_full, &tm_k_8, kj, kh); advance(kj, kh);
+        if (T > 1) { load_half(&tm_k_full, &tm_k_8, kj, kh); advance(kj, kh); }
+        for (int t = 0; t < T; ++t) {
+          load_half(&tm_v_full, &tm_v_8, vj, vh); advance(vj, vh);
+          if (t + 2 < T) { load_half(&tm_k_full, &tm_k_8, kj, kh); advance(kj, kh); }
         }
       }
     } else if (warp == 5) {
       // =============================== MMA issuer ===============================
       if (lane == 0) {
-        constexpr uint32_t idesc_qk = idesc_bf16(128, BLK, 0);
+        constexpr uint32_t idesc_qk = idesc_bf16(128, HALF, 0);
         constexpr uint32_t idesc_pv = idesc_bf16(128, D, 1);
-        mbar_wait(bar(BAR_Q_FULL), 0);
-        for (int j = 0; j < n_tiles; ++j) {
-          const uint32_t ph = j & 1;
-          // S = Q K^T
-          mbar_wait(bar(BAR_K_FULL), ph);
+        int c = 0;                                   // running consume index: slot = c % 4
+        auto issue_qk = [&](int t) {
+          const int slot = c & (kStages - 1);
+          const uint32_t sK = sRing + slot * L::kStage;
+          mbar_wait(bar(BAR_FULL + slot), (c >> 2) & 1);
           tc_fence_after();
 #pragma unroll
           for (int kk = 0; kk < D / 16; ++kk) {
             const uint64_t da = smem_desc_sw128(sQ + (kk >> 2) * L::kQChunk + (kk & 3) * 32, 16, 1024);
             const uint64_t db = smem_desc_sw128(sK + (kk >> 2) * L::kKVChunk + (kk & 3) * 32, 16, 1024);
-            mma_ss(tmem, da, db, idesc_qk, kk > 0);
+            mma_ss(tmem + (t & 1) * kSbCol, da, db, idesc_qk, kk > 0);
           }
-          mma_commit(bar(BAR_K_EMPTY));
-          mma_commit(bar(BAR_S_FULL));
-          // O += P V
-          mbar_wait(bar(BAR_V_FULL), ph);
-          mbar_wait(bar(BAR_P_FULL), ph);
+          mma_commit(bar(BAR_EMPTY + slot));
+          mma_commit(bar(BAR_S_FULL + (t & 1)));
+          ++c;
+        };
+        mbar_wait(bar(BAR_Q_FULL), 0);
+        issue_qk(0);
+        if (T > 1) issue_qk(1);
+        for (int t = 0; t < T; ++t) {
+          // O += P(t) V(t)
+          const int slot = c & (kStages - 1);
+          const uint32_t sV = sRing + slot * L::kStage;
+          mbar_wait(bar(BAR_FULL + slot), (c >> 2) & 1);
+          mbar_wait(bar(BAR_P_FULL + (t & 1)), (t >> 1) & 1);
           tc_fence_after();
 #pragma unroll
-          for (int kk = 0; kk < BLK / 16; ++kk) {
+          for (int kk = 0; kk < HALF / 16; ++kk) {
             const uint64_t db = smem_desc_sw128(sV + kk * 2048, L::kKVChunk, 1024);
-            mma_ts(tmem + kOCol, tmem + kk * 8, db, idesc_pv, (j > 0 || kk > 0) ? 1u : 0u);
+            mma_ts(tmem + kOCol, tmem + (t & 1) * kSbCol + kk * 8, db, idesc_pv, (t > 0 || kk > 0) ? 1u : 0u);
           }
-          mma_commit(bar(BAR_V_EMPTY));
-          if (j == n_tiles - 1) mma_commit(bar(BAR_O_FULL));
+          mma_commit(bar(BAR_EMPTY + slot));
+          mma_commit(bar(BAR_PV_DONE));
+          if (t == T - 1) mma_commit(bar(BAR_O_FULL));
+          ++c;
+          if (t + 2 < T) issue_qk(t + 2);
         }
       }
       __syncwarp();
     } else {
-      // =============================== softmax / correction / epilogue ===============================
+      // =============================== softmax / lazy correction / epilogue ===============================
       const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
       const int row = warp * 32 + lane;                // query row inside the tile == TMEM lane
       float m_used = 0.f, l = 0.f;
-      const int tail_cur = L_cur - (Nc - 1) * BLK, tail_hist = L_hist - (M - 1) * BLK;
+      int j = 0, hh = 0;
 
-      for (int j = 0; j < n_tiles; ++j) {
-        int valid = BLK;
-        if (j < Nc) { if (j == Nc - 1) valid = tail_cur; }
-        else if (sel_at(j - Nc) == M - 1) valid = tail_hist;
+      for (int t = 0; t < T; ++t) {
+        const int tv = tile_valid(j);
+        const int hv = min(HALF, tv - hh * HALF);      // valid key columns of this half-tile (> 0)
+        if (hh == 0 && tv > HALF) hh = 1;
+        else { ++j; hh = 0; }
+        const uint32_t s_addr = tmem + lane_base + (t & 1) * kSbCol;
 
-        mbar_wait(bar(BAR_S_FULL), j & 1);
+        mbar_wait(bar(BAR_S_FULL + (t & 1)), (t >> 1) & 1);
         tc_fence_after();
-        uint32_t s[BLK];
+        uint32_t s[HALF];
 #pragma unroll
-        for (int c = 0; c < BLK / 32; ++c) tmem_ld32(tmem + lane_base + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&s[c * 32]));
+        for (int c = 0; c < HALF / 32; ++c) tmem_ld32(s_addr + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&s[c * 32]));
         tc_wait_ld();
-        if (valid < BLK) {                             // padded key columns -> -inf (warp-uniform branch)
+        if (hv < HALF) {                               // padded key columns -> -inf (warp-uniform branch)
 #pragma unroll
-          for (int c = 0; c < BLK; ++c) if (c >= valid) s[c] = 0xff800000u;
+          for (int c = 0; c < HALF; ++c) if (c >= hv) s[c] = 0xff800000u;
         }
-        float mx = __uint_as_float(s[0]);
+        float mx0 = __uint_as_float(s[0]), mx1 = __uint_as_float(s[1]), mx2 = __uint_as_float(s[2]), mx3 = __uint_as_float(s[3]);
 #pragma unroll
-        for (int c = 1; c < BLK; ++c) mx = fmaxf(mx, __uint_as_float(s[c]));
-        const float m_new = mx * p.scale_log2;
+        for (int c = 4; c < HALF; c += 4) {
+          mx0 = fmaxf(mx0, __uint_as_float(s[c]));
+          mx1 = fmaxf(mx1, __uint_as_float(s[c + 1]));
+          mx2 = fmaxf(mx2, __uint_as_float(s[c + 2]));
+          mx3 = fmaxf(mx3, __uint_as_float(s[c + 3]));
+        }
+        const float m_new = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * p.scale_log2;
 
-        // lazy rescale: move the reference maximum only when the row maximum grew by more than 2^8
+        // lazy rescale: the reference maximum only moves when the row maximum grew by more than 2^8
         bool need = false;
-        if (j == 0) m_used = m_new;
+        if (t == 0) m_used = m_new;
         else need = m_new > m_used + kRescaleThreshold;
         if (__ballot_sync(0xffffffffu, need)) {
+          // O is being accumulated by PV(t-1): wait for it (PV(t-2) is known complete, so the parity is unambiguous)
+          mbar_wait(bar(BAR_PV_DONE), (t - 1) & 1);
+          tc_fence_after();
           const float f = need ? ex2_approx(m_used - m_new) : 1.0f;
           if (need) { m_used = m_new; l *= f; }
 #pragma unroll
@@ -221,23 +278,25 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
 
         // P = exp2(s*scale - m_used), row sum in fp32, bf16 pairs packed low = even column
         const float neg_m = -m_used;
-        float sum0 = 0.f, sum1 = 0.f;
-        uint32_t pk[BLK / 2];
+        float sum0 = 0.f, sum1 = 0.f, sum2 = 0.f, sum3 = 0.f;
+        uint32_t pk[HALF / 2];
 #pragma unroll
-        for (int c = 0; c < BLK / 2; ++c) {
-          const float p0 = ex2_approx(fmaf(__uint_as_float(s[2 * c]), p.scale_log2, neg_m));
-          const float p1 = ex2_approx(fmaf(__uint_as_float(s[2 * c + 1]), p.scale_log2, neg_m));
-          sum0 += p0;
-          sum1 += p1;
-          pk[c] = pack_bf16x2(p0, p1);
+        for (int c = 0; c < HALF / 4; ++c) {
+          const float p0 = ex2_approx(fmaf(__uint_as_float(s[4 * c]), p.scale_log2, neg_m));
+          const float p1 = ex2_approx(fmaf(__uint_as_float(s[4 * c + 1]), p.scale_log2, neg_m));
+          const float p2 = ex2_approx(fmaf(__uint_as_float(s[4 * c + 2]), p.scale_log2, neg_m));
+          const float p3 = ex2_approx(fmaf(__uint_as_float(s[4 * c + 3]), p.scale_log2, neg_m));
+          sum0 += p0; sum1 += p1; sum2 += p2; sum3 += p3;
+          pk[2 * c] = pack_bf16x2(p0, p1);
+          pk[2 * c + 1] = pack_bf16x2(p2, p3);
         }
-        l += sum0 + sum1;
-#pragma unroll
-        for (int c = 0; c < BLK / 64; ++c) tmem_st32(tmem + lane_base + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&pk[c * 32]));
+        l += (sum0 + sum1) + (sum2 + sum3);
+        if constexpr (HALF == 64) tmem_st32(s_addr, *reinterpret_cast<uint32_t(*)[32]>(&pk[0]));
+        else tmem_st16(s_addr, pk);
         tc_wait_st();
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(bar(BAR_P_FULL));
+        if (lane == 0) mbar_arrive(bar(BAR_P_FULL + (t & 1)));
       }
 
       // epilogue: O / l -> bf16, stored in linear token order (no untile pass)

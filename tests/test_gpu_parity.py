@@ -152,3 +152,18 @@ def test_constant_v_and_nan_in_unused_pages(P):
     o = buf.o.float().cpu()
     assert torch.isfinite(o).all() and (o - 0.75).abs().max() < 1e-2
     assert torch.isfinite(buf.scores.cpu()[..., :prob.M(0)]).all()
+
+
+def test_growing_row_maximum_exercises_lazy_rescale(P):
+    """Keys whose logits grow from tile to tile (later pages scaled up) force the kernel's lazy-rescale path
+    (reference maximum moved, O rescaled in TMEM while earlier P.V products are still being accumulated)."""
+    spec = W.spec_small(name="small-rescale", H=2, d=128, block=128, frame_tokens=200, n_cur_frames=3, n_pages=12,
+                        n_mem=(2,), n_win=(3,), density=Fraction(1, 1))
+    prob = W.build(spec)
+    frames = [int(x) for x in prob.frame_idx]
+    # attention order is chunk blocks first, then history blocks ascending: make each later frame "louder"
+    order = frames[-spec.n_cur_frames:] + frames[:-spec.n_cur_frames]
+    for rank, pg in enumerate(order):
+        prob.k_cache[pg] = (prob.k_cache[pg].float() * (1.0 + 1.5 * rank)).to(torch.bfloat16)
+    excused, mx, mean = P.full_parity(prob)
+    print(f"small-rescale: excused={excused} max-abs={mx:.3g} mean-abs={mean:.3g}")
