@@ -34,6 +34,7 @@ template <int D>
 __global__ void __launch_bounds__(kPoolThreads) li_pool_kernel(const SelectParams p, const BatchMeta meta) {
   constexpr int TPR = D / 8;                 // threads per row (16-byte loads)
   constexpr int RPP = kPoolThreads / TPR;    // rows per pass
+  constexpr int kMaxIter = 128 / RPP;        // passes for the largest block (128 rows); bf16 zero adds nothing
   __shared__ float red[RPP][D];
   const int h = blockIdx.y, b = blockIdx.z;
   const int r0 = threadIdx.x / TPR, cofs = (threadIdx.x % TPR) * 8;
@@ -46,8 +47,14 @@ __global__ void __launch_bounds__(kPoolThreads) li_pool_kernel(const SelectParam
     const int t0 = i * p.blk;
     nvalid = min(p.blk, p.Lq - t0);
     const uint16_t *base = p.q + b * p.q_sb + h * p.q_sh + (int64_t)t0 * p.q_st + cofs;
-#pragma unroll 4
-    for (int r = r0; r < nvalid; r += RPP) add_bf16x8(acc, ldg_stream(base + (int64_t)r * p.q_st));
+    uint4 v[kMaxIter];
+#pragma unroll
+    for (int it = 0; it < kMaxIter; ++it) {
+      const int r = r0 + it * RPP;
+      v[it] = r < nvalid ? ldg_stream(base + (int64_t)r * p.q_st) : make_uint4(0, 0, 0, 0);
+    }
+#pragma unroll
+    for (int it = 0; it < kMaxIter; ++it) add_bf16x8(acc, v[it]);
     out = p.qbar + (((int64_t)b * p.H + h) * p.Nqb + i) * D;
   } else {
     const int m = blockIdx.x - p.Nqb;
@@ -59,14 +66,21 @@ __global__ void __launch_bounds__(kPoolThreads) li_pool_kernel(const SelectParam
     nvalid = min(p.blk, L_hist - t0);
     const uint16_t *base = p.k_cache + h * p.kv_sh + cofs;
     const int32_t *pages = p.frame_idx + foff;
-#pragma unroll 4
-    for (int r = r0; r < nvalid; r += RPP) {
-      const int t = t0 + r;
-      const int pg = t / p.T_f;
-      const int row = t - pg * p.T_f;
-      const int page = __ldg(pages + pg);
-      add_bf16x8(acc, ldg_stream(base + page * p.kv_sp + row * p.kv_st));
+    uint4 v[kMaxIter];
+#pragma unroll
+    for (int it = 0; it < kMaxIter; ++it) {
+      const int r = r0 + it * RPP;
+      v[it] = make_uint4(0, 0, 0, 0);
+      if (r < nvalid) {
+        const int t = t0 + r;
+        const int pg = t / p.T_f;
+        const int row = t - pg * p.T_f;
+        const int page = __ldg(pages + pg);
+        v[it] = ldg_stream(base + page * p.kv_sp + row * p.kv_st);
+      }
     }
+#pragma unroll
+    for (int it = 0; it < kMaxIter; ++it) add_bf16x8(acc, v[it]);
     out = p.kbar + (((int64_t)b * p.H + h) * p.Mmax + m) * D;
   }
 
@@ -108,37 +122,54 @@ __global__ void __launch_bounds__(kRowsPerCta * 32) li_score_topk_kernel(const S
   }
   __syncthreads();
 
-  // ---- scores (Eq. 10): warp per historical block m, lanes across d ----
+  // ---- scores (Eq. 10): a warp takes 4 historical blocks at a time, lanes across d; the 4 x 8 partial dot
+  // products per lane are summed over the 32 lanes by a transposing butterfly (31 shuffles instead of 160),
+  // after which lane (mm*8 + g) holds the finished score of block m0+mm for query row g ----
   constexpr int EPL = D / 32;                                // elements per lane (4 or 2)
   float qreg[kRowsPerCta][EPL];
 #pragma unroll
   for (int g = 0; g < kRowsPerCta; ++g)
 #pragma unroll
     for (int e = 0; e < EPL; ++e) qreg[g][e] = sq[g * D + lane * EPL + e];
-  for (int m = warp; m < M; m += kRowsPerCta) {
-    const float *kr = p.kbar + (bh * p.Mmax + m) * D + lane * EPL;
-    float kv[EPL];
+  for (int m0 = warp * 4; m0 < M; m0 += kRowsPerCta * 4) {
+    float kv[4][EPL];
 #pragma unroll
-    for (int e = 0; e < EPL; ++e) kv[e] = kr[e];
-    float dot[kRowsPerCta];
-#pragma unroll
-    for (int g = 0; g < kRowsPerCta; ++g) {
-      float s = 0.f;
-#pragma unroll
-      for (int e = 0; e < EPL; ++e) s = fmaf(qreg[g][e], kv[e], s);
-      dot[g] = s;
+    for (int mm = 0; mm < 4; ++mm) {
+      const int m = min(m0 + mm, M - 1);
+      const float *kr = p.kbar + (bh * p.Mmax + m) * D + lane * EPL;
+      if constexpr (EPL == 4) {
+        const float4 t = *reinterpret_cast<const float4 *>(kr);
+        kv[mm][0] = t.x; kv[mm][1] = t.y; kv[mm][2] = t.z; kv[mm][3] = t.w;
+      } else {
+        const float2 t = *reinterpret_cast<const float2 *>(kr);
+        kv[mm][0] = t.x; kv[mm][1] = t.y;
+      }
     }
+    float v[32];
 #pragma unroll
-    for (int off = 16; off > 0; off >>= 1)
+    for (int mm = 0; mm < 4; ++mm)
 #pragma unroll
-      for (int g = 0; g < kRowsPerCta; ++g) dot[g] += __shfl_xor_sync(0xffffffffu, dot[g], off);
-    if (lane < kRowsPerCta && i0 + lane < p.Nqb) {
-      float s = 0.f;
+      for (int g = 0; g < kRowsPerCta; ++g) {
+        float a = 0.f;
 #pragma unroll
-      for (int g = 0; g < kRowsPerCta; ++g) if (g == lane) s = dot[g];
-      s = s * p.inv_sqrt_d + 0.0f;                          // -0 -> +0 so that equal scores have equal keys
-      skey[lane * p.Mmax + m] = order_key(s);
-      if (p.scores != nullptr) p.scores[(bh * p.Nqb + i0 + lane) * p.score_pitch + m] = s;
+        for (int e = 0; e < EPL; ++e) a = fmaf(qreg[g][e], kv[mm][e], a);
+        v[mm * 8 + g] = a;
+      }
+#pragma unroll
+    for (int w = 16; w >= 1; w >>= 1) {
+      const bool up = (lane & w) != 0;                       // this lane keeps the upper half of the values
+#pragma unroll
+      for (int x = 0; x < w; ++x) {
+        const float keep = up ? v[x + w] : v[x];
+        const float send = up ? v[x] : v[x + w];
+        v[x] = keep + __shfl_xor_sync(0xffffffffu, send, w);
+      }
+    }
+    const int m = m0 + (lane >> 3), g = lane & 7;
+    if (m < M && i0 + g < p.Nqb) {
+      const float sc = v[0] * p.inv_sqrt_d + 0.0f;           // -0 -> +0 so that equal scores have equal keys
+      skey[g * p.Mmax + m] = order_key(sc);
+      if (p.scores != nullptr) p.scores[(bh * p.Nqb + i0 + g) * p.score_pitch + m] = sc;
     }
   }
   __syncthreads();
