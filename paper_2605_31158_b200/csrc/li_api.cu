@@ -45,6 +45,7 @@ bool encode_map(CUtensorMap *tm, const void *base, int d, int64_t n1, int64_t n2
 }
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+inline size_t mpad(int m) { return m > 0 ? (size_t)((m + 31) & ~31) : 32; }   // row pitch of the transposed kbar
 
 struct Derived {
   int Nqb, Nc, Mmax;
@@ -90,8 +91,9 @@ int check_problem(const li_problem *p, Derived *dv) {
 
 size_t ws_bytes(const li_problem *p, const Derived &dv) {
   const size_t qbar = align256((size_t)p->B * p->H * dv.Nqb * p->d * 4);
-  const size_t kbar = align256((size_t)p->B * p->H * (dv.Mmax > 0 ? dv.Mmax : 1) * p->d * 4);
-  return qbar + kbar;
+  const size_t kbar = align256((size_t)p->B * p->H * mpad(dv.Mmax) * p->d * 4);
+  const size_t keys = align256((size_t)p->B * p->H * dv.Nqb * (dv.Mmax > 0 ? dv.Mmax : 1) * 4);
+  return qbar + kbar + keys;
 }
 
 }  // namespace
@@ -122,8 +124,6 @@ int li_block_select(const li_problem *p, const int32_t *top_k_host, int32_t kmax
     if (k > kmax) return LI_ERR_INVALID_ARG;
     dv.meta.top_k[b] = k;
   }
-  // dynamic shared memory of the score/top-k kernel: 8 rows of Mmax keys + 8 pooled query rows
-  if ((size_t)8 * dv.Mmax * 4 + (size_t)8 * p->d * 4 > 200 * 1024) return LI_ERR_UNSUPPORTED;
 
   li::SelectParams sp;
   std::memset(&sp, 0, sizeof(sp));
@@ -135,6 +135,8 @@ int li_block_select(const li_problem *p, const int32_t *top_k_host, int32_t kmax
   sp.frame_idx = p->frame_idx;
   sp.qbar = (float *)workspace;
   sp.kbar = (float *)((char *)workspace + align256((size_t)p->B * p->H * dv.Nqb * p->d * 4));
+  sp.Mp = (int32_t)mpad(dv.Mmax);
+  sp.keys = (uint32_t *)((char *)sp.kbar + align256((size_t)p->B * p->H * mpad(dv.Mmax) * p->d * 4));
   sp.sel_idx = sel_idx; sp.sel_cnt = sel_cnt; sp.scores = scores_opt;
   sp.inv_sqrt_d = 1.0f / std::sqrt((float)p->d);
   int64_t n = 0;

@@ -15,14 +15,15 @@ struct BatchMeta {
 };
 
 struct SelectParams {
-  int32_t B, H, Lq, d, T_f, blk, n_cur, Nqb, Mmax, kmax, score_pitch;
+  int32_t B, H, Lq, d, T_f, blk, n_cur, Nqb, Mmax, Mp, kmax, score_pitch;   // Mp = Mmax rounded up to 32
   const uint16_t *q;
   int64_t q_sb, q_sh, q_st;
   const uint16_t *k_cache;
   int64_t kv_sp, kv_sh, kv_st;
   const int32_t *frame_idx;
   float *qbar;     // [B,H,Nqb,d]
-  float *kbar;     // [B,H,Mmax,d]
+  float *kbar;     // [B,H,d,Mp]  (transposed: channel-major)
+  uint32_t *keys;  // [B,H,Nqb,Mmax] order-preserving score keys
   int32_t *sel_idx;
   int32_t *sel_cnt;
   float *scores;   // optional

@@ -2,9 +2,9 @@
 //   kernel 1  li_pool_kernel       : block means of Q and of the historical K (K rows fetched through the
 //                                    frame-index list, in place).  HBM-bound streaming reduction: every Q and
 //                                    historical-K byte is read exactly once with 16-byte loads.
-//   kernel 2  li_score_topk_kernel : scores qbar_i . kbar_m / sqrt(d) (fp32) and the per-row top-k by an
-//                                    MSB-first radix select on order-preserving keys; ties -> lowest block index;
-//                                    indices written ascending.
+//   kernel 2  li_score_kernel      : scores qbar_i . kbar_m / sqrt(d) (fp32) -> order-preserving uint32 keys.
+//   kernel 3  li_topk_kernel       : per-row top-k by an MSB-first radix select on the keys; ties -> lowest block
+//                                    index; indices written ascending.
 #include "li_internal.h"
 
 namespace li {
@@ -41,6 +41,7 @@ __global__ void __launch_bounds__(kPoolThreads) li_pool_kernel(const SelectParam
   float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
   int nvalid;
   float *out;
+  int out_stride = 1;
 
   if ((int)blockIdx.x < p.Nqb) {
     const int i = blockIdx.x;
@@ -81,7 +82,8 @@ __global__ void __launch_bounds__(kPoolThreads) li_pool_kernel(const SelectParam
     }
 #pragma unroll
     for (int it = 0; it < kMaxIter; ++it) add_bf16x8(acc, v[it]);
-    out = p.kbar + (((int64_t)b * p.H + h) * p.Mmax + m) * D;
+    out = p.kbar + ((int64_t)b * p.H + h) * D * p.Mp + m;          // kbar is stored TRANSPOSED: [B,H,d,Mp]
+    out_stride = p.Mp;
   }
 
 #pragma unroll
@@ -91,122 +93,161 @@ __global__ void __launch_bounds__(kPoolThreads) li_pool_kernel(const SelectParam
     float s = 0.f;
 #pragma unroll
     for (int r = 0; r < RPP; ++r) s += red[r][threadIdx.x];
-    out[threadIdx.x] = s / (float)nvalid;    // Eq. 9: true cardinality |Q_i|, |K_m|
+    out[(int64_t)threadIdx.x * out_stride] = s / (float)nvalid;    // Eq. 9: true cardinality |Q_i|, |K_m|
   }
 }
 
-constexpr int kRowsPerCta = 8;               // query-block rows per CTA == warps per CTA
+constexpr int kRowsPerWarp = 8;              // query-block rows scored together by one warp
+constexpr int kKeysPerLane = 16;             // top-k register fast path covers M <= 512 historical blocks
+constexpr int kTopkWarps = 8;                // rows (warps) per CTA of the top-k kernel
 
 __device__ __forceinline__ uint32_t order_key(float s) {
   const uint32_t u = __float_as_uint(s);
   return (u & 0x80000000u) ? ~u : (u | 0x80000000u);   // unsigned order == float order
 }
 
-// grid = (ceil(Nqb / 8), H, B), 256 threads, dynamic smem = 8 * Mmax * 4 bytes (keys) + 8 * D * 4 (qbar rows)
+// Scores (Eq. 10).  grid = (ceil(Mmax/32), ceil(Nqb/8), B*H), ONE warp per CTA (thousands of independent warps:
+// the work is latency-bound, so it is spread as thinly as possible).  lane = one historical block m; the lane walks
+// its pooled key row (16-byte read-only loads) against 8 pooled query rows broadcast from shared memory: 8
+// independent fp32 FMA chains, no cross-lane reduction.  Output: order-preserving keys [B,H,Nqb,Mmax] (+ scores).
 template <int D>
-__global__ void __launch_bounds__(kRowsPerCta * 32) li_score_topk_kernel(const SelectParams p, const BatchMeta meta) {
-  extern __shared__ uint32_t sm[];
-  float *sq = reinterpret_cast<float *>(sm);                 // [8][D]
-  uint32_t *skey = sm + kRowsPerCta * D;                     // [8][Mmax]
-  const int h = blockIdx.y, b = blockIdx.z;
+__global__ void __launch_bounds__(32) li_score_kernel(const SelectParams p, const BatchMeta meta) {
+  __shared__ __align__(16) float sq[kRowsPerWarp * D];
+  const int lane = threadIdx.x;
+  const int bh = blockIdx.z, b = bh / p.H;
+  const int i0 = blockIdx.y * kRowsPerWarp;
+  const int n_hist = meta.frame_off[b + 1] - meta.frame_off[b] - p.n_cur;
+  const int M = (n_hist * p.T_f + p.blk - 1) / p.blk;
+  const int m = blockIdx.x * 32 + lane;
+  if ((int)blockIdx.x * 32 >= M) return;
+
+  // kbar is [B,H,d,Mp] (written transposed by the pool kernel): for a fixed channel the 32 lanes read 32
+  // consecutive floats = one 128-byte line.  Lanes past M read padding and their results are dropped.
+  const float *kT = p.kbar + (int64_t)bh * D * p.Mp + m;
+  constexpr int CH = 16;                                     // channels per batch of loads
+  float kv[CH];
+#pragma unroll
+  for (int c = 0; c < CH; ++c) kv[c] = __ldg(kT + (int64_t)c * p.Mp);   // in flight while the q rows are staged
+  for (int t = lane; t < kRowsPerWarp * D / 4; t += 32) {
+    const int g = t / (D / 4);
+    reinterpret_cast<float4 *>(sq)[t] =
+        (i0 + g < p.Nqb) ? __ldg(reinterpret_cast<const float4 *>(p.qbar + ((int64_t)bh * p.Nqb + i0) * D) + t)
+                         : make_float4(0.f, 0.f, 0.f, 0.f);
+  }
+  __syncwarp();
+
+  float acc[kRowsPerWarp];
+#pragma unroll
+  for (int g = 0; g < kRowsPerWarp; ++g) acc[g] = 0.f;
+#pragma unroll
+  for (int c0 = 0; c0 < D; c0 += CH) {
+    float nx[CH];
+    if (c0 + CH < D) {
+#pragma unroll
+      for (int c = 0; c < CH; ++c) nx[c] = __ldg(kT + (int64_t)(c0 + CH + c) * p.Mp);
+    }
+#pragma unroll
+    for (int c = 0; c < CH; c += 4) {
+#pragma unroll
+      for (int g = 0; g < kRowsPerWarp; ++g) {
+        const float4 qv = *reinterpret_cast<const float4 *>(sq + g * D + c0 + c);
+        acc[g] = fmaf(qv.x, kv[c], acc[g]);
+        acc[g] = fmaf(qv.y, kv[c + 1], acc[g]);
+        acc[g] = fmaf(qv.z, kv[c + 2], acc[g]);
+        acc[g] = fmaf(qv.w, kv[c + 3], acc[g]);
+      }
+    }
+    if (c0 + CH < D) {
+#pragma unroll
+      for (int c = 0; c < CH; ++c) kv[c] = nx[c];
+    }
+  }
+  if (m < M) {
+#pragma unroll
+    for (int g = 0; g < kRowsPerWarp; ++g) {
+      if (i0 + g < p.Nqb) {
+        const float sc = acc[g] * p.inv_sqrt_d + 0.0f;       // -0 -> +0 so that equal scores have equal keys
+        p.keys[((int64_t)bh * p.Nqb + i0 + g) * p.Mmax + m] = order_key(sc);
+        if (p.scores != nullptr) p.scores[((int64_t)bh * p.Nqb + i0 + g) * p.score_pitch + m] = sc;
+      }
+    }
+  }
+}
+
+// Top_k (Eq. 10).  One warp per (call, head, query block) row; grid = ceil(B*H*Nqb / 8) CTAs of 8 warps.
+// MSB-first radix select of the k-th largest key, then one ordered pass that emits, ascending, every block above
+// the threshold plus the lowest-index blocks equal to it.
+__global__ void __launch_bounds__(kTopkWarps * 32) li_topk_kernel(const SelectParams p, const BatchMeta meta) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int i0 = blockIdx.x * kRowsPerCta;
+  const int64_t row = (int64_t)blockIdx.x * kTopkWarps + warp;
+  if (row >= (int64_t)p.B * p.H * p.Nqb) return;
+  const int b = (int)(row / ((int64_t)p.H * p.Nqb));
   const int n_hist = meta.frame_off[b + 1] - meta.frame_off[b] - p.n_cur;
   const int M = (n_hist * p.T_f + p.blk - 1) / p.blk;
   const int k = min(meta.top_k[b], M);
-  const int64_t bh = (int64_t)b * p.H + h;
-
-  for (int t = threadIdx.x; t < kRowsPerCta * D; t += blockDim.x) {
-    const int g = t / D, c = t % D;
-    sq[t] = (i0 + g < p.Nqb) ? p.qbar[(bh * p.Nqb + i0 + g) * D + c] : 0.f;
-  }
-  __syncthreads();
-
-  // ---- scores (Eq. 10): a warp takes 4 historical blocks at a time, lanes across d; the 4 x 8 partial dot
-  // products per lane are summed over the 32 lanes by a transposing butterfly (31 shuffles instead of 160),
-  // after which lane (mm*8 + g) holds the finished score of block m0+mm for query row g ----
-  constexpr int EPL = D / 32;                                // elements per lane (4 or 2)
-  float qreg[kRowsPerCta][EPL];
-#pragma unroll
-  for (int g = 0; g < kRowsPerCta; ++g)
-#pragma unroll
-    for (int e = 0; e < EPL; ++e) qreg[g][e] = sq[g * D + lane * EPL + e];
-  for (int m0 = warp * 4; m0 < M; m0 += kRowsPerCta * 4) {
-    float kv[4][EPL];
-#pragma unroll
-    for (int mm = 0; mm < 4; ++mm) {
-      const int m = min(m0 + mm, M - 1);
-      const float *kr = p.kbar + (bh * p.Mmax + m) * D + lane * EPL;
-      if constexpr (EPL == 4) {
-        const float4 t = *reinterpret_cast<const float4 *>(kr);
-        kv[mm][0] = t.x; kv[mm][1] = t.y; kv[mm][2] = t.z; kv[mm][3] = t.w;
-      } else {
-        const float2 t = *reinterpret_cast<const float2 *>(kr);
-        kv[mm][0] = t.x; kv[mm][1] = t.y;
-      }
-    }
-    float v[32];
-#pragma unroll
-    for (int mm = 0; mm < 4; ++mm)
-#pragma unroll
-      for (int g = 0; g < kRowsPerCta; ++g) {
-        float a = 0.f;
-#pragma unroll
-        for (int e = 0; e < EPL; ++e) a = fmaf(qreg[g][e], kv[mm][e], a);
-        v[mm * 8 + g] = a;
-      }
-#pragma unroll
-    for (int w = 16; w >= 1; w >>= 1) {
-      const bool up = (lane & w) != 0;                       // this lane keeps the upper half of the values
-#pragma unroll
-      for (int x = 0; x < w; ++x) {
-        const float keep = up ? v[x + w] : v[x];
-        const float send = up ? v[x] : v[x + w];
-        v[x] = keep + __shfl_xor_sync(0xffffffffu, send, w);
-      }
-    }
-    const int m = m0 + (lane >> 3), g = lane & 7;
-    if (m < M && i0 + g < p.Nqb) {
-      const float sc = v[0] * p.inv_sqrt_d + 0.0f;           // -0 -> +0 so that equal scores have equal keys
-      skey[g * p.Mmax + m] = order_key(sc);
-      if (p.scores != nullptr) p.scores[(bh * p.Nqb + i0 + g) * p.score_pitch + m] = sc;
-    }
-  }
-  __syncthreads();
-
-  // ---- Top_k (Eq. 10): warp per query-block row ----
-  const int i = i0 + warp;
-  if (i >= p.Nqb) return;
-  const uint32_t *key = skey + warp * p.Mmax;
-  int32_t *out = p.sel_idx + (bh * p.Nqb + i) * p.kmax;
-  if (lane == 0) p.sel_cnt[bh * p.Nqb + i] = k;
+  const uint32_t *key = p.keys + row * p.Mmax;
+  int32_t *out = p.sel_idx + row * p.kmax;
+  if (lane == 0) p.sel_cnt[row] = k;
   if (k > 0) {
     // T = k-th largest key: build it MSB first, keeping count(key >= T) >= k
     uint32_t T = 0;
-    for (int bit = 31; bit >= 0; --bit) {
-      const uint32_t cand = T | (1u << bit);
-      int c = 0;
-      for (int m = lane; m < M; m += 32) c += key[m] >= cand;
-      c = __reduce_add_sync(0xffffffffu, c);
-      if (c >= k) T = cand;
-    }
     int c_gt = 0;
-    for (int m = lane; m < M; m += 32) c_gt += key[m] > T;
-    c_gt = __reduce_add_sync(0xffffffffu, c_gt);
-    int need_eq = k - c_gt;                                  // ties at the threshold: lowest index first
-    int pos = 0;
-    for (int m0 = 0; m0 < M; m0 += 32) {
-      const int m = m0 + lane;
-      const uint32_t kv = m < M ? key[m] : 0u;
-      const bool gt = m < M && kv > T;
-      const bool eq = m < M && kv == T;
-      const uint32_t eq_mask = __ballot_sync(0xffffffffu, eq);
-      const uint32_t lt = (1u << lane) - 1u;
-      const bool take = gt || (eq && __popc(eq_mask & lt) < need_eq);
-      const uint32_t take_mask = __ballot_sync(0xffffffffu, take);
-      if (take) out[pos + __popc(take_mask & lt)] = m;
-      pos += __popc(take_mask);
-      need_eq -= min(need_eq, __popc(eq_mask));
+    if (M <= 32 * kKeysPerLane) {
+      // fast path: each lane keeps its keys (block m = lane + 32*x) in registers; absent blocks get key 0,
+      // which is below every real key (order_key never returns 0 for a non-NaN score)
+      uint32_t kr[kKeysPerLane];
+#pragma unroll
+      for (int x = 0; x < kKeysPerLane; ++x) kr[x] = (lane + 32 * x < M) ? key[lane + 32 * x] : 0u;
+      for (int bit = 31; bit >= 0; --bit) {
+        const uint32_t cand = T | (1u << bit);
+        int c = 0;
+#pragma unroll
+        for (int x = 0; x < kKeysPerLane; ++x) c += kr[x] >= cand;
+        c = __reduce_add_sync(0xffffffffu, c);
+        if (c >= k) T = cand;
+      }
+#pragma unroll
+      for (int x = 0; x < kKeysPerLane; ++x) c_gt += kr[x] > T;
+      c_gt = __reduce_add_sync(0xffffffffu, c_gt);
+      int need_eq = k - c_gt;                                // ties at the threshold: lowest index first
+      int pos = 0;
+#pragma unroll
+      for (int x = 0; x < kKeysPerLane; ++x) {
+        const bool gt = kr[x] > T;
+        const bool eq = kr[x] == T && T != 0u;
+        const uint32_t eq_mask = __ballot_sync(0xffffffffu, eq);
+        const uint32_t lt = (1u << lane) - 1u;
+        const bool take = gt || (eq && __popc(eq_mask & lt) < need_eq);
+        const uint32_t take_mask = __ballot_sync(0xffffffffu, take);
+        if (take) out[pos + __popc(take_mask & lt)] = lane + 32 * x;
+        pos += __popc(take_mask);
+        need_eq -= min(need_eq, __popc(eq_mask));
+      }
+    } else {
+      for (int bit = 31; bit >= 0; --bit) {
+        const uint32_t cand = T | (1u << bit);
+        int c = 0;
+        for (int m = lane; m < M; m += 32) c += key[m] >= cand;
+        c = __reduce_add_sync(0xffffffffu, c);
+        if (c >= k) T = cand;
+      }
+      for (int m = lane; m < M; m += 32) c_gt += key[m] > T;
+      c_gt = __reduce_add_sync(0xffffffffu, c_gt);
+      int need_eq = k - c_gt;
+      int pos = 0;
+      for (int m0 = 0; m0 < M; m0 += 32) {
+        const int m = m0 + lane;
+        const uint32_t kv = m < M ? key[m] : 0u;
+        const bool gt = m < M && kv > T;
+        const bool eq = m < M && kv == T;
+        const uint32_t eq_mask = __ballot_sync(0xffffffffu, eq);
+        const uint32_t lt = (1u << lane) - 1u;
+        const bool take = gt || (eq && __popc(eq_mask & lt) < need_eq);
+        const uint32_t take_mask = __ballot_sync(0xffffffffu, take);
+        if (take) out[pos + __popc(take_mask & lt)] = m;
+        pos += __popc(take_mask);
+        need_eq -= min(need_eq, __popc(eq_mask));
+      }
     }
   }
   for (int t = k + lane; t < p.kmax; t += 32) out[t] = -1;
@@ -221,20 +262,18 @@ int launch_select(const SelectParams &sp, const BatchMeta &meta, cudaStream_t st
     if (e != cudaSuccess) return (int)e;
     if (n_launches) *n_launches += 1;
   }
+  if (sp.Mmax > 0) {
+    dim3 grid((sp.Mmax + 31) / 32, (sp.Nqb + kRowsPerWarp - 1) / kRowsPerWarp, sp.B * sp.H);
+    if (sp.d == 128) li_score_kernel<128><<<grid, 32, 0, st>>>(sp, meta);
+    else li_score_kernel<64><<<grid, 32, 0, st>>>(sp, meta);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return (int)e;
+    if (n_launches) *n_launches += 1;
+  }
   {
-    dim3 grid((sp.Nqb + kRowsPerCta - 1) / kRowsPerCta, sp.H, sp.B);
-    const size_t smem = (size_t)kRowsPerCta * (sp.Mmax > 0 ? sp.Mmax : 1) * 4 + (size_t)kRowsPerCta * sp.d * 4;
-    cudaError_t e;
-    if (sp.d == 128) {
-      e = cudaFuncSetAttribute(li_score_topk_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-      if (e != cudaSuccess) return (int)e;
-      li_score_topk_kernel<128><<<grid, kRowsPerCta * 32, smem, st>>>(sp, meta);
-    } else {
-      e = cudaFuncSetAttribute(li_score_topk_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-      if (e != cudaSuccess) return (int)e;
-      li_score_topk_kernel<64><<<grid, kRowsPerCta * 32, smem, st>>>(sp, meta);
-    }
-    e = cudaGetLastError();
+    const int64_t rows = (int64_t)sp.B * sp.H * sp.Nqb;
+    li_topk_kernel<<<(unsigned)((rows + kTopkWarps - 1) / kTopkWarps), kTopkWarps * 32, 0, st>>>(sp, meta);
+    cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return (int)e;
     if (n_launches) *n_launches += 1;
   }

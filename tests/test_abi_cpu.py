@@ -70,8 +70,9 @@ def make_problem(**over):
 def test_workspace_bytes_and_validation(L):
     p, fo = make_problem()
     ws = L.li_workspace_bytes(ctypes.byref(p), 8)
-    # qbar [1,2,4,64] fp32 + kbar [1,2,12,64] fp32, each rounded up to 256 B
-    assert ws == 2 * 4 * 64 * 4 + 2 * 12 * 64 * 4
+    # qbar [1,2,4,64] fp32 + kbar [1,2,64,32] fp32 (transposed, M padded to 32) + score keys [1,2,4,12] u32,
+    # each rounded up to 256 B
+    assert ws == 2 * 4 * 64 * 4 + 2 * 64 * 32 * 4 + 512
     tk = np.asarray([8], dtype=np.int32)
 
     def select(prob, kmax=8, ws_ptr=0x50000, ws_bytes=ws, sel=0x60000, cnt=0x70000):
