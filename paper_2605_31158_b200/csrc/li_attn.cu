@@ -78,14 +78,10 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
   const int M = (L_hist + BLK - 1) / BLK;
   const int Nc = (L_cur + BLK - 1) / BLK;
   const int64_t row_id = ((int64_t)b * p.H + h) * p.Nqb + i;
-  const int cnt = p.sel_cnt[row_id];
-  const int32_t *sel_row = p.sel_idx + row_id * p.kmax;
-  const int n_tiles = Nc + cnt;
   const int valid_q = min(BLK, p.Lq - i * BLK);
   const int tail_cur = L_cur - (Nc - 1) * BLK, tail_hist = L_hist - (M - 1) * BLK;
 
-  // ---- one-time setup ----
-  for (int t = threadIdx.x; t < cnt && t < kSelCap; t += blockDim.x) sSel[t] = sel_row[t];
+  // ---- one-time setup (independent of the previous kernel: overlaps its tail under PDL) ----
   if (warp == 4 && lane == 0) {
     tma_prefetch_desc(&tm_q);
     tma_prefetch_desc(&tm_k_full);
@@ -100,6 +96,11 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
     tmem_alloc(smem_u32(tmem_slot), kTmemCols);
     tmem_relinquish();
   }
+  asm volatile("griddepcontrol.wait;" ::: "memory");     // sel_idx / sel_cnt come from li_block_select (PDL)
+  const int cnt = p.sel_cnt[row_id];
+  const int32_t *sel_row = p.sel_idx + row_id * p.kmax;
+  const int n_tiles = Nc + cnt;
+  for (int t = threadIdx.x; t < cnt && t < kSelCap; t += blockDim.x) sSel[t] = sel_row[t];
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -350,8 +351,18 @@ static int launch_one(const AttnParams &ap, const BatchMeta &meta, const CUtenso
   constexpr int smem = AttnSmem<D, BLK>::kTotal;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   if (e != cudaSuccess) return (int)e;
-  dim3 grid(ap.Nqb, ap.H, ap.B);
-  kern<<<grid, 192, smem, st>>>(ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8);
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(ap.Nqb, ap.H, ap.B);
+  cfg.blockDim = dim3(192);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  e = cudaLaunchKernelEx(&cfg, kern, ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8);
+  if (e != cudaSuccess) return (int)e;
   return (int)cudaGetLastError();
 }
 

@@ -9,6 +9,11 @@
 
 namespace li {
 
+// programmatic dependent launch: let the next kernel of the stream start its prologue early / wait for the
+// previous kernel's results
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 __device__ __forceinline__ uint4 ldg_stream(const void *p) {
   uint4 r;
   asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
@@ -36,6 +41,7 @@ __global__ void __launch_bounds__(kPoolThreads) li_pool_kernel(const SelectParam
   constexpr int RPP = kPoolThreads / TPR;    // rows per pass
   constexpr int kMaxIter = 128 / RPP;        // passes for the largest block (128 rows); bf16 zero adds nothing
   __shared__ float red[RPP][D];
+  pdl_launch_dependents();
   const int h = blockIdx.y, b = blockIdx.z;
   const int r0 = threadIdx.x / TPR, cofs = (threadIdx.x % TPR) * 8;
   float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
@@ -120,6 +126,8 @@ __global__ void __launch_bounds__(32) li_score_kernel(const SelectParams p, cons
   const int M = (n_hist * p.T_f + p.blk - 1) / p.blk;
   const int m = blockIdx.x * 32 + lane;
   if ((int)blockIdx.x * 32 >= M) return;
+  pdl_launch_dependents();
+  pdl_wait();                                              // qbar / kbar come from li_pool_kernel
 
   // kbar is [B,H,d,Mp] (written transposed by the pool kernel): for a fixed channel the 32 lanes read 32
   // consecutive floats = one 128-byte line.  Lanes past M read padding and their results are dropped.
@@ -181,6 +189,8 @@ __global__ void __launch_bounds__(kTopkWarps * 32) li_topk_kernel(const SelectPa
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int64_t row = (int64_t)blockIdx.x * kTopkWarps + warp;
   if (row >= (int64_t)p.B * p.H * p.Nqb) return;
+  pdl_launch_dependents();
+  pdl_wait();                                              // keys come from li_score_kernel
   const int b = (int)(row / ((int64_t)p.H * p.Nqb));
   const int n_hist = meta.frame_off[b + 1] - meta.frame_off[b] - p.n_cur;
   const int M = (n_hist * p.T_f + p.blk - 1) / p.blk;
@@ -262,18 +272,30 @@ int launch_select(const SelectParams &sp, const BatchMeta &meta, cudaStream_t st
     if (e != cudaSuccess) return (int)e;
     if (n_launches) *n_launches += 1;
   }
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
   if (sp.Mmax > 0) {
-    dim3 grid((sp.Mmax + 31) / 32, (sp.Nqb + kRowsPerWarp - 1) / kRowsPerWarp, sp.B * sp.H);
-    if (sp.d == 128) li_score_kernel<128><<<grid, 32, 0, st>>>(sp, meta);
-    else li_score_kernel<64><<<grid, 32, 0, st>>>(sp, meta);
-    cudaError_t e = cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((sp.Mmax + 31) / 32, (sp.Nqb + kRowsPerWarp - 1) / kRowsPerWarp, sp.B * sp.H);
+    cfg.blockDim = dim3(32);
+    cfg.stream = st;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cudaError_t e = sp.d == 128 ? cudaLaunchKernelEx(&cfg, li_score_kernel<128>, sp, meta)
+                                : cudaLaunchKernelEx(&cfg, li_score_kernel<64>, sp, meta);
     if (e != cudaSuccess) return (int)e;
     if (n_launches) *n_launches += 1;
   }
   {
     const int64_t rows = (int64_t)sp.B * sp.H * sp.Nqb;
-    li_topk_kernel<<<(unsigned)((rows + kTopkWarps - 1) / kTopkWarps), kTopkWarps * 32, 0, st>>>(sp, meta);
-    cudaError_t e = cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)((rows + kTopkWarps - 1) / kTopkWarps));
+    cfg.blockDim = dim3(kTopkWarps * 32);
+    cfg.stream = st;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cudaError_t e = cudaLaunchKernelEx(&cfg, li_topk_kernel, sp, meta);
     if (e != cudaSuccess) return (int)e;
     if (n_launches) *n_launches += 1;
   }
