@@ -24,6 +24,10 @@ constexpr int kSbCol = 64;
 constexpr int kOCol = 128;
 constexpr int kStages = 4;
 constexpr float kRescaleThreshold = 8.0f;   // log2 units: P stays <= 2^8 between lazy rescales
+#ifndef LI_EMU_OF_4
+#define LI_EMU_OF_4 0
+#endif
+constexpr int kEmuOf4 = LI_EMU_OF_4;        // of every 4 column pairs, how many use the FMA-pipe exp2
 
 template <int D, int BLK>
 struct AttnSmem {
@@ -277,21 +281,32 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
           }
         }
 
-        // P = exp2(s*scale - m_used), row sum in fp32, bf16 pairs packed low = even column
-        const float neg_m = -m_used;
-        float sum0 = 0.f, sum1 = 0.f, sum2 = 0.f, sum3 = 0.f;
+        // P = exp2(s*scale - m_used), row sum in fp32, bf16 pairs packed low = even column.  kEmuOf4 of every 4
+        // column pairs take the FMA-pipe exp2 (li_ptx.cuh), the others the MUFU, so that both pipes stay busy.
+        const uint64_t sc2 = pack2(p.scale_log2, p.scale_log2), nm2 = pack2(-m_used, -m_used);
+        uint64_t sum_a = pack2(0.f, 0.f), sum_b = pack2(0.f, 0.f);
         uint32_t pk[HALF / 2];
 #pragma unroll
-        for (int c = 0; c < HALF / 4; ++c) {
-          const float p0 = ex2_approx(fmaf(__uint_as_float(s[4 * c]), p.scale_log2, neg_m));
-          const float p1 = ex2_approx(fmaf(__uint_as_float(s[4 * c + 1]), p.scale_log2, neg_m));
-          const float p2 = ex2_approx(fmaf(__uint_as_float(s[4 * c + 2]), p.scale_log2, neg_m));
-          const float p3 = ex2_approx(fmaf(__uint_as_float(s[4 * c + 3]), p.scale_log2, neg_m));
-          sum0 += p0; sum1 += p1; sum2 += p2; sum3 += p3;
-          pk[2 * c] = pack_bf16x2(p0, p1);
-          pk[2 * c + 1] = pack_bf16x2(p2, p3);
+        for (int c = 0; c < HALF / 2; ++c) {
+          const uint64_t x2 = fma2(pack2(__uint_as_float(s[2 * c]), __uint_as_float(s[2 * c + 1])), sc2, nm2);
+          float p0, p1;
+          if ((c & 3) < kEmuOf4) {
+            exp2_emulated2(x2, p0, p1);
+          } else {
+            float x0, x1;
+            unpack2(x2, x0, x1);
+            p0 = ex2_approx(x0);
+            p1 = ex2_approx(x1);
+          }
+          if (c & 1) sum_b = add2(sum_b, pack2(p0, p1));
+          else sum_a = add2(sum_a, pack2(p0, p1));
+          pk[c] = pack_bf16x2(p0, p1);
         }
-        l += (sum0 + sum1) + (sum2 + sum3);
+        {
+          float a0, a1;
+          unpack2(add2(sum_a, sum_b), a0, a1);
+          l += a0 + a1;
+        }
         if constexpr (HALF == 64) tmem_st32(s_addr, *reinterpret_cast<uint32_t(*)[32]>(&pk[0]));
         else tmem_st16(s_addr, pk);
         tc_wait_st();

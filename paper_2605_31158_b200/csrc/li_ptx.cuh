@@ -155,6 +155,25 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t *r) {
       : "memory");
 }
 
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t *r) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+        "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+      : "r"(taddr)
+      : "memory");
+}
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t *r) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr),
+               "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])
+               : "memory");
+}
+// named barrier among `nthreads` threads of the CTA (id 1..15; 0 is __syncthreads)
+__device__ __forceinline__ void named_bar_sync(uint32_t id, uint32_t nthreads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
 // 64-bit shared-memory matrix descriptor, SWIZZLE_128B, Blackwell version field = 1.
 //   bits [0,14)  start address >> 4      bits [16,30) leading-dimension byte offset >> 4
 //   bits [32,46) stride-dimension byte offset >> 4      bits [46,48) version = 1      bits [61,64) layout = 2
@@ -183,6 +202,48 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
   uint32_t r;
   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
   return r;
+}
+
+// ----------------------------------------------------------------------------- packed fp32x2 (sm_100: FFMA2 / FADD2)
+__device__ __forceinline__ uint64_t pack2(float lo, float hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void unpack2(uint64_t v, float &lo, float &hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
+  uint64_t r;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+
+// 2^x for a pair of x <= ~8 on the FMA/ALU pipes instead of the MUFU (which, at 16 ex2/clk/SM, costs as many cycles
+// per attention tile as the tensor core does): Cody-Waite split x = n + f, n = round(x) taken from the mantissa of
+// x + 1.5*2^23, f in [-0.5, 0.5], 2^f by a degree-3 minimax polynomial (max relative error 7.5e-5, far below the
+// bf16 rounding of P), 2^n applied by adding n to the exponent field.
+__device__ __forceinline__ void exp2_emulated2(uint64_t x2, float &p0, float &p1) {
+  float x0, x1;
+  unpack2(x2, x0, x1);
+  x2 = pack2(fmaxf(x0, -126.0f), fmaxf(x1, -126.0f));          // keep the exponent arithmetic in range
+  const uint64_t magic = pack2(12582912.0f, 12582912.0f), neg_magic = pack2(-12582912.0f, -12582912.0f);
+  const uint64_t t2 = add2(x2, magic);                           // low mantissa bits of t = round(x)
+  const uint64_t n2 = add2(t2, neg_magic);                       // round(x) as a float (exact)
+  const uint64_t f2 = fma2(n2, pack2(-1.0f, -1.0f), x2);         // x - round(x)
+  uint64_t q2 = fma2(pack2(0.05517132207751274f, 0.05517132207751274f), f2, pack2(0.24261054396629333f, 0.24261054396629333f));
+  q2 = fma2(q2, f2, pack2(0.6932609677314758f, 0.6932609677314758f));
+  q2 = fma2(q2, f2, pack2(0.9999281167984009f, 0.9999281167984009f));
+  float q0, q1, t0, t1;
+  unpack2(q2, q0, q1);
+  unpack2(t2, t0, t1);
+  p0 = __uint_as_float(__float_as_uint(q0) + (__float_as_uint(t0) << 23));
+  p1 = __uint_as_float(__float_as_uint(q1) + (__float_as_uint(t1) << 23));
 }
 
 }  // namespace li
