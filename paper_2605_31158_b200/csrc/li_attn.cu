@@ -8,9 +8,10 @@
 // S(t), and O += P(t) V(t) is issued as soon as P(t) is written.  Tensor-core issue order:
 //     QK(0) QK(1) | PV(0) QK(2) | PV(1) QK(3) | ...      (K/V half-tiles are loaded in exactly this order
 //                                                         into a 4-slot shared-memory ring)
-//   warps 0-3 : softmax + lazy correction + epilogue; warp w owns TMEM lanes 32w..32w+31 (one query row per thread)
-//   warp 4    : TMA producer (one elected lane): Q once, then the K/V half-tiles
-//   warp 5    : TMEM allocation and the single-thread tcgen05.mma issuer
+//   warps 0-7 : softmax + lazy correction + epilogue; warps w and w+4 own TMEM lanes 32w..32w+31 and split the
+//               columns of every half-tile (two threads per query row: the softmax is issue/latency-bound)
+//   warp 8    : TMA producer (one elected lane): Q once, then the K/V half-tiles
+//   warp 9    : TMEM allocation and the single-thread tcgen05.mma issuer
 // TMEM (256 columns): [0,HALF) S_a, [64,64+HALF) S_b (fp32; P in bf16 overlays the first HALF/2 columns of its S
 // buffer once S has been read), [128,128+D) O.
 #include "li_internal.h"
@@ -23,6 +24,7 @@ constexpr int kTmemCols = 256;
 constexpr int kSbCol = 64;
 constexpr int kOCol = 128;
 constexpr int kStages = 4;
+constexpr int kSoftmaxWarps = 8, kProducerWarp = 8, kMmaWarp = 9, kThreads = 320;
 constexpr float kRescaleThreshold = 8.0f;   // log2 units: P stays <= 2^8 between lazy rescales
 #ifndef LI_EMU_OF_4
 #define LI_EMU_OF_4 0
@@ -39,7 +41,8 @@ struct AttnSmem {
   static constexpr int kOffQ = 0;
   static constexpr int kOffRing = kQ;
   static constexpr int kOffSel = kQ + kStages * kStage;
-  static constexpr int kOffBar = kOffSel + kSelCap * 4;
+  static constexpr int kOffXch = kOffSel + kSelCap * 4;   // row-max / row-sum exchange between the two threads of a row
+  static constexpr int kOffBar = kOffXch + 6 * 128 * 4;
   static constexpr int kTotal = kOffBar + 256 + 1024;  // + barriers + slack for 1024-B alignment
 };
 
@@ -55,7 +58,7 @@ enum {
 };
 
 template <int D, int BLK>
-__global__ void __launch_bounds__(192, 2)
+__global__ void __launch_bounds__(kThreads, 2)
 li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_constant__ CUtensorMap tm_q,
                       const __grid_constant__ CUtensorMap tm_k_full, const __grid_constant__ CUtensorMap tm_k_8,
                       const __grid_constant__ CUtensorMap tm_v_full, const __grid_constant__ CUtensorMap tm_v_8) {
@@ -66,6 +69,7 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
   uint8_t *smem = smem_raw + (smem_base - smem_u32(smem_raw));
   const uint32_t sQ = smem_base + L::kOffQ, sRing = smem_base + L::kOffRing;
   int32_t *sSel = reinterpret_cast<int32_t *>(smem + L::kOffSel);
+  volatile float *sXch = reinterpret_cast<volatile float *>(smem + L::kOffXch);
   const uint32_t bar0 = smem_base + L::kOffBar;
   uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + L::kOffBar + 8 * BAR_COUNT);
   auto bar = [&](int i) { return bar0 + 8u * i; };
@@ -86,17 +90,17 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
   const int tail_cur = L_cur - (Nc - 1) * BLK, tail_hist = L_hist - (M - 1) * BLK;
 
   // ---- one-time setup (independent of the previous kernel: overlaps its tail under PDL) ----
-  if (warp == 4 && lane == 0) {
+  if (warp == kProducerWarp && lane == 0) {
     tma_prefetch_desc(&tm_q);
     tma_prefetch_desc(&tm_k_full);
     tma_prefetch_desc(&tm_v_full);
     tma_prefetch_desc(&tm_k_8);
     tma_prefetch_desc(&tm_v_8);
-    for (int k = 0; k < BAR_COUNT; ++k) mbar_init(bar(k), (k == BAR_P_FULL || k == BAR_P_FULL + 1) ? 4 : 1);
+    for (int k = 0; k < BAR_COUNT; ++k) mbar_init(bar(k), (k == BAR_P_FULL || k == BAR_P_FULL + 1) ? 8 : 1);
     mbar_fence_init();
     fence_proxy_async();
   }
-  if (warp == 5) {
+  if (warp == kMmaWarp) {
     tmem_alloc(smem_u32(tmem_slot), kTmemCols);
     tmem_relinquish();
   }
@@ -122,7 +126,7 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
   if (cnt > 0 && sel_at(cnt - 1) == M - 1 && tail_hist <= HALF) --T;
 
   if (T > 0) {
-    if (warp == 4) {
+    if (warp == kProducerWarp) {
       // =============================== TMA producer ===============================
       if (lane == 0) {
         mbar_arrive_expect_tx(bar(BAR_Q_FULL), BLK * D * 2);
@@ -182,7 +186,7 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
           if (t + 2 < T) { load_half(&tm_k_full, &tm_k_8, kj, kh); advance(kj, kh); }
         }
       }
-    } else if (warp == 5) {
+    } else if (warp == kMmaWarp) {
       // =============================== MMA issuer ===============================
       if (lane == 0) {
         constexpr uint32_t idesc_qk = idesc_bf16(128, HALF, 0);
@@ -228,66 +232,76 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
       __syncwarp();
     } else {
       // =============================== softmax / lazy correction / epilogue ===============================
-      const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
-      const int row = warp * 32 + lane;                // query row inside the tile == TMEM lane
+      // Two threads per query row: warps w and w+4 own the same TMEM lanes 32w..32w+31 and split every half-tile's
+      // columns (and, in the epilogue, O's columns) in two.  The pair agrees on the row maximum through shared memory
+      // and a 64-thread named barrier; each keeps a partial row sum.
+      const int sw = warp & 3, part = warp >> 2;
+      const uint32_t lane_base = (uint32_t)(sw * 32) << 16;
+      const int row = sw * 32 + lane;                  // query row inside the tile == TMEM lane
+      constexpr int CW = HALF / 2;                     // S columns per thread per half-tile
       float m_used = 0.f, l = 0.f;
       int j = 0, hh = 0;
 
       for (int t = 0; t < T; ++t) {
         const int tv = tile_valid(j);
-        const int hv = min(HALF, tv - hh * HALF);      // valid key columns of this half-tile (> 0)
+        const int hv = min(HALF, tv - hh * HALF) - part * CW;   // valid columns among this thread's CW (may be <= 0)
         if (hh == 0 && tv > HALF) hh = 1;
         else { ++j; hh = 0; }
         const uint32_t s_addr = tmem + lane_base + (t & 1) * kSbCol;
 
         mbar_wait(bar(BAR_S_FULL + (t & 1)), (t >> 1) & 1);
         tc_fence_after();
-        uint32_t s[HALF];
-#pragma unroll
-        for (int c = 0; c < HALF / 32; ++c) tmem_ld32(s_addr + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&s[c * 32]));
+        uint32_t s[CW];
+        if constexpr (CW == 32) tmem_ld32(s_addr + part * CW, *reinterpret_cast<uint32_t(*)[32]>(&s[0]));
+        else tmem_ld16(s_addr + part * CW, s);
         tc_wait_ld();
-        if (hv < HALF) {                               // padded key columns -> -inf (warp-uniform branch)
+        if (hv < CW) {                                 // padded key columns -> -inf (warp-uniform branch)
 #pragma unroll
-          for (int c = 0; c < HALF; ++c) if (c >= hv) s[c] = 0xff800000u;
+          for (int c = 0; c < CW; ++c) if (c >= hv) s[c] = 0xff800000u;
         }
         float mx0 = __uint_as_float(s[0]), mx1 = __uint_as_float(s[1]), mx2 = __uint_as_float(s[2]), mx3 = __uint_as_float(s[3]);
 #pragma unroll
-        for (int c = 4; c < HALF; c += 4) {
+        for (int c = 4; c < CW; c += 4) {
           mx0 = fmaxf(mx0, __uint_as_float(s[c]));
           mx1 = fmaxf(mx1, __uint_as_float(s[c + 1]));
           mx2 = fmaxf(mx2, __uint_as_float(s[c + 2]));
           mx3 = fmaxf(mx3, __uint_as_float(s[c + 3]));
         }
-        const float m_new = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * p.scale_log2;
+        const float mx_mine = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
+        sXch[((t & 1) * 2 + part) * 128 + row] = mx_mine;
+        named_bar_sync(1 + sw, 64);
+        const float m_new = fmaxf(mx_mine, sXch[((t & 1) * 2 + (part ^ 1)) * 128 + row]) * p.scale_log2;
 
         // lazy rescale: the reference maximum only moves when the row maximum grew by more than 2^8
         bool need = false;
         if (t == 0) m_used = m_new;
         else need = m_new > m_used + kRescaleThreshold;
         if (__ballot_sync(0xffffffffu, need)) {
-          // O is being accumulated by PV(t-1): wait for it (PV(t-2) is known complete, so the parity is unambiguous)
+          // O is being accumulated by PV(t-1): wait for it (PV(t-2) is known complete, so the parity is unambiguous).
+          // Both warps of a pair take this branch together (same m_new); each rescales half of O's columns.
           mbar_wait(bar(BAR_PV_DONE), (t - 1) & 1);
           tc_fence_after();
           const float f = need ? ex2_approx(m_used - m_new) : 1.0f;
           if (need) { m_used = m_new; l *= f; }
-#pragma unroll
-          for (int c = 0; c < D / 32; ++c) {
-            uint32_t o[32];
-            tmem_ld32(tmem + lane_base + kOCol + c * 32, o);
+#pragma unroll 1
+          for (int c = 0; c < D / 32; ++c) {             // rare path: small chunks keep the register footprint low
+            uint32_t o[16];
+            const uint32_t o_addr = tmem + lane_base + kOCol + part * (D / 2) + c * 16;
+            tmem_ld16(o_addr, o);
             tc_wait_ld();
 #pragma unroll
-            for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * f);
-            tmem_st32(tmem + lane_base + kOCol + c * 32, o);
+            for (int e = 0; e < 16; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * f);
+            tmem_st16(o_addr, o);
           }
         }
 
         // P = exp2(s*scale - m_used), row sum in fp32, bf16 pairs packed low = even column.  kEmuOf4 of every 4
-        // column pairs take the FMA-pipe exp2 (li_ptx.cuh), the others the MUFU, so that both pipes stay busy.
+        // column pairs take the FMA-pipe exp2 (li_ptx.cuh), the others the MUFU.
         const uint64_t sc2 = pack2(p.scale_log2, p.scale_log2), nm2 = pack2(-m_used, -m_used);
         uint64_t sum_a = pack2(0.f, 0.f), sum_b = pack2(0.f, 0.f);
-        uint32_t pk[HALF / 2];
+        uint32_t pk[CW / 2];
 #pragma unroll
-        for (int c = 0; c < HALF / 2; ++c) {
+        for (int c = 0; c < CW / 2; ++c) {
           const uint64_t x2 = fma2(pack2(__uint_as_float(s[2 * c]), __uint_as_float(s[2 * c + 1])), sc2, nm2);
           float p0, p1;
           if ((c & 3) < kEmuOf4) {
@@ -307,24 +321,27 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
           unpack2(add2(sum_a, sum_b), a0, a1);
           l += a0 + a1;
         }
-        if constexpr (HALF == 64) tmem_st32(s_addr, *reinterpret_cast<uint32_t(*)[32]>(&pk[0]));
-        else tmem_st16(s_addr, pk);
+        if constexpr (CW == 32) tmem_st16(s_addr + part * (CW / 2), pk);
+        else tmem_st8(s_addr + part * (CW / 2), pk);
         tc_wait_st();
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(bar(BAR_P_FULL + (t & 1)));
       }
 
-      // epilogue: O / l -> bf16, stored in linear token order (no untile pass)
+      // epilogue: O / l -> bf16, stored in linear token order (no untile pass); each thread of a pair stores half a row
+      sXch[(4 + part) * 128 + row] = l;
+      named_bar_sync(1 + sw, 64);
+      l += sXch[(4 + (part ^ 1)) * 128 + row];
       mbar_wait(bar(BAR_O_FULL), 0);
       tc_fence_after();
       const float inv_l = 1.0f / l;
       const bool live = row < valid_q;
-      uint16_t *orow = p.o + (((int64_t)b * p.H + h) * p.Lq + (int64_t)i * BLK + row) * D;
+      uint16_t *orow = p.o + (((int64_t)b * p.H + h) * p.Lq + (int64_t)i * BLK + row) * D + part * (D / 2);
 #pragma unroll
-      for (int c = 0; c < D / 32; ++c) {
+      for (int c = 0; c < D / 64; ++c) {
         uint32_t o[32];
-        tmem_ld32(tmem + lane_base + kOCol + c * 32, o);
+        tmem_ld32(tmem + lane_base + kOCol + part * (D / 2) + c * 32, o);
         tc_wait_ld();
         if (live) {
 #pragma unroll
@@ -338,7 +355,7 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
           }
         }
       }
-      if (live && p.lse != nullptr)
+      if (part == 0 && live && p.lse != nullptr)
         p.lse[((int64_t)b * p.H + h) * p.Lq + (int64_t)i * BLK + row] = (m_used + log2f(l)) * 0.6931471805599453f;
     }
   } else {
@@ -355,7 +372,7 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
 
   tc_fence_before();
   __syncthreads();
-  if (warp == 5) tmem_dealloc(tmem, kTmemCols);
+  if (warp == kMmaWarp) tmem_dealloc(tmem, kTmemCols);
 }
 
 template <int D, int BLK>
@@ -371,7 +388,7 @@ static int launch_one(const AttnParams &ap, const BatchMeta &meta, const CUtenso
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(ap.Nqb, ap.H, ap.B);
-  cfg.blockDim = dim3(192);
+  cfg.blockDim = dim3(kThreads);
   cfg.dynamicSmemBytes = smem;
   cfg.stream = st;
   cfg.attrs = attr;
