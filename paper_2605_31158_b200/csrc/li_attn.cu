@@ -2,29 +2,32 @@
 // (Eq. 11), K/V tiles fetched IN PLACE from the frame-paged cache by TMA with the page
 // as a tensor coordinate (replaces the paper's KV-Prep / Untile-Scatter copies).
 //
-// One CTA = one query block (BLK query rows, padded to the 128-row UMMA tile) of one (call, head); two CTAs per SM.
-// Every attended KV block is processed as two HALF-tiles of HALF = BLK/2 keys, software-pipelined inside the CTA:
-// S is double-buffered in TMEM, so the tensor core computes S(t+1) = Q K(t+1)^T while the softmax warps work on
-// S(t), and O += P(t) V(t) is issued as soon as P(t) is written.  Tensor-core issue order:
-//     QK(0) QK(1) | PV(0) QK(2) | PV(1) QK(3) | ...      (K/V half-tiles are loaded in exactly this order
-//                                                         into a 4-slot shared-memory ring)
-//   warps 0-7 : softmax + lazy correction + epilogue; warps w and w+4 own TMEM lanes 32w..32w+31 and split the
-//               columns of every half-tile (two threads per query row: the softmax is issue/latency-bound)
-//   warp 8    : TMA producer (one elected lane): Q once, then the K/V half-tiles
-//   warp 9    : TMEM allocation and the single-thread tcgen05.mma issuer
-// TMEM (256 columns): [0,HALF) S_a, [64,64+HALF) S_b (fp32; P in bf16 overlays the first HALF/2 columns of its S
-// buffer once S has been read), [128,128+D) O.
+// One CTA per SM = one query block (BLK query rows, padded to the 128-row UMMA tile) of one (call, head).
+// What bounds this kernel on B200 is, in this order: shared-memory bandwidth (128 B/clk/SM), the MUFU (16 ex2/clk/SM)
+// and the tensor pipe, all three within 1.5x of each other for d = 128.  Hence:
+//   * Q lives in TENSOR MEMORY (written once through registers with tcgen05.st) and is the A operand of S = Q K^T,
+//     so the tensor core never re-reads Q from shared memory; shared memory only sees each K/V byte twice
+//     (TMA write + one MMA read).
+//   * Every attended KV block is processed as two HALF-tiles of HALF = BLK/2 keys; S is TRIPLE-buffered in TMEM, the
+//     tensor core runs up to three half-tiles ahead of the softmax warps, which therefore never wait for it:
+//         QK(0) QK(1) QK(2) | PV(0) QK(3) | PV(1) QK(4) | ...   (K/V half-tiles are TMA-loaded in exactly this order
+//                                                                into an 8-slot shared-memory ring)
+//   * HALF/16 threads per query row (16 S columns each): the softmax is latency-bound, more warps hide it.
+//   warps 0..4*NPART-1 : softmax + lazy correction + epilogue; warp w owns TMEM lanes 32(w%4).. and column part w/4
+//   next warp          : TMA producer (one elected lane)
+//   last warp          : TMEM allocation and the single-thread tcgen05.mma issuer
+// TMEM (512 columns): [0,D/2) Q (bf16 pairs), [64,..) [128,..) [192,..) S buffers (fp32; P in bf16 overlays the first
+// HALF/2 columns of its S buffer once S has been read), [256,256+D) O.
 #include "li_internal.h"
 #include "li_ptx.cuh"
 
 namespace li {
 
 constexpr int kSelCap = 1024;       // selected-block indices staged in shared memory (rest read from global)
-constexpr int kTmemCols = 256;
-constexpr int kSbCol = 64;
-constexpr int kOCol = 128;
-constexpr int kStages = 4;
-constexpr int kSoftmaxWarps = 8, kProducerWarp = 8, kMmaWarp = 9, kThreads = 320;
+constexpr int kTmemCols = 512;
+constexpr int kQCol = 0, kSCol = 64, kSStride = 64, kOCol = 256;
+constexpr int kStages = 8;          // K/V half-tile ring
+constexpr int kSBufs = 3;
 constexpr float kRescaleThreshold = 8.0f;   // log2 units: P stays <= 2^8 between lazy rescales
 #ifndef LI_EMU_OF_4
 #define LI_EMU_OF_4 0
@@ -32,42 +35,44 @@ constexpr float kRescaleThreshold = 8.0f;   // log2 units: P stays <= 2^8 betwee
 constexpr int kEmuOf4 = LI_EMU_OF_4;        // of every 4 column pairs, how many use the FMA-pipe exp2
 
 template <int D, int BLK>
-struct AttnSmem {
+struct AttnCfg {
   static constexpr int HALF = BLK / 2;
-  static constexpr int kQChunk = 128 * 128;            // bytes of one 64-column chunk of the 128-row Q tile
+  static constexpr int CW = 16;                        // S columns per softmax thread per half-tile
+  static constexpr int NPART = HALF / CW;              // threads per query row (4 for BLK=128, 2 for BLK=64)
+  static constexpr int kSoftmaxWarps = 4 * NPART;
+  static constexpr int kProducerWarp = kSoftmaxWarps, kMmaWarp = kSoftmaxWarps + 1;
+  static constexpr int kThreads = (kSoftmaxWarps + 2) * 32;
   static constexpr int kKVChunk = HALF * 128;          // bytes of one 64-column chunk of a K or V half-tile
-  static constexpr int kQ = (D / 64) * kQChunk;
   static constexpr int kStage = (D / 64) * kKVChunk;
-  static constexpr int kOffQ = 0;
-  static constexpr int kOffRing = kQ;
-  static constexpr int kOffSel = kQ + kStages * kStage;
-  static constexpr int kOffXch = kOffSel + kSelCap * 4;   // row-max / row-sum exchange between the two threads of a row
-  static constexpr int kOffBar = kOffXch + 6 * 128 * 4;
-  static constexpr int kTotal = kOffBar + 256 + 1024;  // + barriers + slack for 1024-B alignment
+  static constexpr int kOffRing = 0;
+  static constexpr int kOffSel = kStages * kStage;
+  static constexpr int kOffXch = kOffSel + kSelCap * 4;              // row-max / row-sum exchange: [3][NPART][128] floats
+  static constexpr int kOffBar = kOffXch + 3 * NPART * 128 * 4;
+  static constexpr int kTotal = kOffBar + 512 + 1024;                // + barriers + slack for 1024-B alignment
 };
 
 enum {
-  BAR_Q_FULL = 0,
-  BAR_FULL = 1,                    // +slot
-  BAR_EMPTY = BAR_FULL + kStages,  // +slot
-  BAR_S_FULL = BAR_EMPTY + kStages,  // +buffer
-  BAR_P_FULL = BAR_S_FULL + 2,       // +buffer
-  BAR_PV_DONE = BAR_P_FULL + 2,
+  BAR_FULL = 0,                        // +slot
+  BAR_EMPTY = BAR_FULL + kStages,      // +slot
+  BAR_S_FULL = BAR_EMPTY + kStages,    // +buffer
+  BAR_P_FULL = BAR_S_FULL + kSBufs,    // +buffer
+  BAR_PV_DONE = BAR_P_FULL + kSBufs,   // +(t & 1)
+  BAR_Q_READY = BAR_PV_DONE + 2,
   BAR_O_FULL,
   BAR_COUNT
 };
 
 template <int D, int BLK>
-__global__ void __launch_bounds__(kThreads, 2)
-li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_constant__ CUtensorMap tm_q,
-                      const __grid_constant__ CUtensorMap tm_k_full, const __grid_constant__ CUtensorMap tm_k_8,
-                      const __grid_constant__ CUtensorMap tm_v_full, const __grid_constant__ CUtensorMap tm_v_8) {
-  using L = AttnSmem<D, BLK>;
-  constexpr int HALF = L::HALF;
+__global__ void __launch_bounds__(AttnCfg<D, BLK>::kThreads, 1)
+li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_constant__ CUtensorMap tm_k_full,
+                      const __grid_constant__ CUtensorMap tm_k_8, const __grid_constant__ CUtensorMap tm_v_full,
+                      const __grid_constant__ CUtensorMap tm_v_8) {
+  using L = AttnCfg<D, BLK>;
+  constexpr int HALF = L::HALF, CW = L::CW, NPART = L::NPART;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   uint8_t *smem = smem_raw + (smem_base - smem_u32(smem_raw));
-  const uint32_t sQ = smem_base + L::kOffQ, sRing = smem_base + L::kOffRing;
+  const uint32_t sRing = smem_base + L::kOffRing;
   int32_t *sSel = reinterpret_cast<int32_t *>(smem + L::kOffSel);
   volatile float *sXch = reinterpret_cast<volatile float *>(smem + L::kOffXch);
   const uint32_t bar0 = smem_base + L::kOffBar;
@@ -90,17 +95,19 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
   const int tail_cur = L_cur - (Nc - 1) * BLK, tail_hist = L_hist - (M - 1) * BLK;
 
   // ---- one-time setup (independent of the previous kernel: overlaps its tail under PDL) ----
-  if (warp == kProducerWarp && lane == 0) {
-    tma_prefetch_desc(&tm_q);
+  if (warp == L::kProducerWarp && lane == 0) {
     tma_prefetch_desc(&tm_k_full);
     tma_prefetch_desc(&tm_v_full);
     tma_prefetch_desc(&tm_k_8);
     tma_prefetch_desc(&tm_v_8);
-    for (int k = 0; k < BAR_COUNT; ++k) mbar_init(bar(k), (k == BAR_P_FULL || k == BAR_P_FULL + 1) ? 8 : 1);
+    for (int k = 0; k < BAR_COUNT; ++k) {
+      const bool by_softmax = (k >= BAR_P_FULL && k < BAR_P_FULL + kSBufs) || k == BAR_Q_READY;
+      mbar_init(bar(k), by_softmax ? L::kSoftmaxWarps : 1);
+    }
     mbar_fence_init();
     fence_proxy_async();
   }
-  if (warp == kMmaWarp) {
+  if (warp == L::kMmaWarp) {
     tmem_alloc(smem_u32(tmem_slot), kTmemCols);
     tmem_relinquish();
   }
@@ -126,15 +133,11 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
   if (cnt > 0 && sel_at(cnt - 1) == M - 1 && tail_hist <= HALF) --T;
 
   if (T > 0) {
-    if (warp == kProducerWarp) {
+    if (warp == L::kProducerWarp) {
       // =============================== TMA producer ===============================
       if (lane == 0) {
-        mbar_arrive_expect_tx(bar(BAR_Q_FULL), BLK * D * 2);
-#pragma unroll
-        for (int c = 0; c < D / 64; ++c) tma_load_4d(sQ + c * L::kQChunk, &tm_q, bar(BAR_Q_FULL), c * 64, i * BLK, h, b);
-
-        int n = 0;                                   // running load index: slot = n % 4
-        // loads HALF rows [t0, t0+HALF) of a region (history or chunk) into ring slot n % 4
+        int n = 0;                                   // running load index: slot = n % kStages
+        // loads HALF rows [t0, t0+HALF) of a region (history or chunk) into the next ring slot
         auto load_half = [&](const CUtensorMap *tm_full, const CUtensorMap *tm_8, int j, int hh) {
           const bool is_cur = j < Nc;
           const int blk = is_cur ? j : sel_at(j - Nc);
@@ -143,7 +146,7 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
           const int t0 = blk * BLK + hh * HALF;
           const int slot = n & (kStages - 1);
           const uint32_t dst = sRing + slot * L::kStage, mb = bar(BAR_FULL + slot);
-          mbar_wait(bar(BAR_EMPTY + slot), ((n >> 2) & 1) ^ 1);
+          mbar_wait(bar(BAR_EMPTY + slot), ((n / kStages) & 1) ^ 1);
           mbar_arrive_expect_tx(mb, HALF * D * 2);
           const int t_last = min(t0 + HALF, region_len) - 1;
           const int pg0 = t0 / p.T_f;
@@ -177,83 +180,102 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
           else { ++j; hh = 0; }
         };
 
-        // load order == consumption order of the MMA warp: K0 K1 | V0 K2 | V1 K3 | ...
+        // load order == consumption order of the MMA warp: K0 K1 K2 | V0 K3 | V1 K4 | ...
         int kj = 0, kh = 0, vj = 0, vh = 0;
-        load_half(&tm_k_full, &tm_k_8, kj, kh); advance(kj, kh);
-        if (T > 1) { load_half(&tm_k_full, &tm_k_8, kj, kh); advance(kj, kh); }
+        for (int t = 0; t < kSBufs && t < T; ++t) { load_half(&tm_k_full, &tm_k_8, kj, kh); advance(kj, kh); }
         for (int t = 0; t < T; ++t) {
           load_half(&tm_v_full, &tm_v_8, vj, vh); advance(vj, vh);
-          if (t + 2 < T) { load_half(&tm_k_full, &tm_k_8, kj, kh); advance(kj, kh); }
+          if (t + kSBufs < T) { load_half(&tm_k_full, &tm_k_8, kj, kh); advance(kj, kh); }
         }
       }
-    } else if (warp == kMmaWarp) {
+    } else if (warp == L::kMmaWarp) {
       // =============================== MMA issuer ===============================
       if (lane == 0) {
         constexpr uint32_t idesc_qk = idesc_bf16(128, HALF, 0);
         constexpr uint32_t idesc_pv = idesc_bf16(128, D, 1);
-        int c = 0;                                   // running consume index: slot = c % 4
-        auto issue_qk = [&](int t) {
+        int c = 0;                                   // running consume index: slot = c % kStages
+        auto issue_qk = [&](int t) {                 // S(t) = Q K(t)^T, Q read from tensor memory
           const int slot = c & (kStages - 1);
           const uint32_t sK = sRing + slot * L::kStage;
-          mbar_wait(bar(BAR_FULL + slot), (c >> 2) & 1);
+          mbar_wait(bar(BAR_FULL + slot), (c / kStages) & 1);
           tc_fence_after();
 #pragma unroll
           for (int kk = 0; kk < D / 16; ++kk) {
-            const uint64_t da = smem_desc_sw128(sQ + (kk >> 2) * L::kQChunk + (kk & 3) * 32, 16, 1024);
             const uint64_t db = smem_desc_sw128(sK + (kk >> 2) * L::kKVChunk + (kk & 3) * 32, 16, 1024);
-            mma_ss(tmem + (t & 1) * kSbCol, da, db, idesc_qk, kk > 0);
+            mma_ts(tmem + kSCol + (t % kSBufs) * kSStride, tmem + kQCol + kk * 8, db, idesc_qk, kk > 0);
           }
           mma_commit(bar(BAR_EMPTY + slot));
-          mma_commit(bar(BAR_S_FULL + (t & 1)));
+          mma_commit(bar(BAR_S_FULL + (t % kSBufs)));
           ++c;
         };
-        mbar_wait(bar(BAR_Q_FULL), 0);
-        issue_qk(0);
-        if (T > 1) issue_qk(1);
+        mbar_wait(bar(BAR_Q_READY), 0);
+        tc_fence_after();
+        for (int t = 0; t < kSBufs && t < T; ++t) issue_qk(t);
         for (int t = 0; t < T; ++t) {
           // O += P(t) V(t)
           const int slot = c & (kStages - 1);
           const uint32_t sV = sRing + slot * L::kStage;
-          mbar_wait(bar(BAR_FULL + slot), (c >> 2) & 1);
-          mbar_wait(bar(BAR_P_FULL + (t & 1)), (t >> 1) & 1);
+          mbar_wait(bar(BAR_FULL + slot), (c / kStages) & 1);
+          mbar_wait(bar(BAR_P_FULL + (t % kSBufs)), (t / kSBufs) & 1);
           tc_fence_after();
 #pragma unroll
           for (int kk = 0; kk < HALF / 16; ++kk) {
             const uint64_t db = smem_desc_sw128(sV + kk * 2048, L::kKVChunk, 1024);
-            mma_ts(tmem + kOCol, tmem + (t & 1) * kSbCol + kk * 8, db, idesc_pv, (t > 0 || kk > 0) ? 1u : 0u);
+            mma_ts(tmem + kOCol, tmem + kSCol + (t % kSBufs) * kSStride + kk * 8, db, idesc_pv, (t > 0 || kk > 0) ? 1u : 0u);
           }
           mma_commit(bar(BAR_EMPTY + slot));
-          mma_commit(bar(BAR_PV_DONE));
+          mma_commit(bar(BAR_PV_DONE + (t & 1)));
           if (t == T - 1) mma_commit(bar(BAR_O_FULL));
           ++c;
-          if (t + 2 < T) issue_qk(t + 2);
+          if (t + kSBufs < T) issue_qk(t + kSBufs);
         }
       }
       __syncwarp();
     } else {
       // =============================== softmax / lazy correction / epilogue ===============================
-      // Two threads per query row: warps w and w+4 own the same TMEM lanes 32w..32w+31 and split every half-tile's
-      // columns (and, in the epilogue, O's columns) in two.  The pair agrees on the row maximum through shared memory
-      // and a 64-thread named barrier; each keeps a partial row sum.
+      // NPART threads per query row: warps w, w+4, ... own the same TMEM lanes 32(w%4).. and split every half-tile's
+      // columns (and Q's / O's columns) among them.  They agree on the row maximum through shared memory and a named
+      // barrier; each keeps a partial row sum.
       const int sw = warp & 3, part = warp >> 2;
       const uint32_t lane_base = (uint32_t)(sw * 32) << 16;
       const int row = sw * 32 + lane;                  // query row inside the tile == TMEM lane
-      constexpr int CW = HALF / 2;                     // S columns per thread per half-tile
+      const bool live = row < valid_q;
+      constexpr int QE = D / NPART;                    // Q / O elements (columns of O) per thread
+
+      // ---- Q -> tensor memory (bf16 pairs, low half = even channel: the A-operand layout, same as P) ----
+      {
+        uint32_t qv[QE / 2];
+        const uint4 *src = reinterpret_cast<const uint4 *>(p.q + b * p.q_sb + h * p.q_sh +
+                                                            ((int64_t)i * BLK + row) * p.q_st + part * QE);
+#pragma unroll
+        for (int c = 0; c < QE / 8; ++c) {
+          const uint4 v = live ? __ldg(src + c) : make_uint4(0, 0, 0, 0);
+          qv[4 * c] = v.x; qv[4 * c + 1] = v.y; qv[4 * c + 2] = v.z; qv[4 * c + 3] = v.w;
+        }
+        const uint32_t q_addr = tmem + lane_base + kQCol + part * (QE / 2);
+        if constexpr (QE / 2 == 32) tmem_st32(q_addr, *reinterpret_cast<uint32_t(*)[32]>(&qv[0]));
+        else if constexpr (QE / 2 == 16) tmem_st16(q_addr, qv);
+        else tmem_st8(q_addr, qv);
+        tc_wait_st();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar(BAR_Q_READY));
+      }
+
       float m_used = 0.f, l = 0.f;
       int j = 0, hh = 0;
-
       for (int t = 0; t < T; ++t) {
         const int tv = tile_valid(j);
         const int hv = min(HALF, tv - hh * HALF) - part * CW;   // valid columns among this thread's CW (may be <= 0)
         if (hh == 0 && tv > HALF) hh = 1;
         else { ++j; hh = 0; }
-        const uint32_t s_addr = tmem + lane_base + (t & 1) * kSbCol;
+        const int u = t % kSBufs;
+        const uint32_t s_addr = tmem + lane_base + kSCol + u * kSStride;
 
-        mbar_wait(bar(BAR_S_FULL + (t & 1)), (t >> 1) & 1);
+        mbar_wait(bar(BAR_S_FULL + u), (t / kSBufs) & 1);
         tc_fence_after();
         uint32_t s[CW];
-        if constexpr (CW == 32) tmem_ld32(s_addr + part * CW, *reinterpret_cast<uint32_t(*)[32]>(&s[0]));
-        else tmem_ld16(s_addr + part * CW, s);
+        tmem_ld16(s_addr + part * CW, s);
         tc_wait_ld();
         if (hv < CW) {                                 // padded key columns -> -inf (warp-uniform branch)
 #pragma unroll
@@ -267,26 +289,29 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
           mx2 = fmaxf(mx2, __uint_as_float(s[c + 2]));
           mx3 = fmaxf(mx3, __uint_as_float(s[c + 3]));
         }
-        const float mx_mine = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
-        sXch[((t & 1) * 2 + part) * 128 + row] = mx_mine;
-        named_bar_sync(1 + sw, 64);
-        const float m_new = fmaxf(mx_mine, sXch[((t & 1) * 2 + (part ^ 1)) * 128 + row]) * p.scale_log2;
+        float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
+        sXch[(u * NPART + part) * 128 + row] = mx;
+        named_bar_sync(1 + sw, NPART * 32);
+#pragma unroll
+        for (int q = 0; q < NPART; ++q) mx = fmaxf(mx, sXch[(u * NPART + q) * 128 + row]);
+        const float m_new = mx * p.scale_log2;
 
         // lazy rescale: the reference maximum only moves when the row maximum grew by more than 2^8
         bool need = false;
         if (t == 0) m_used = m_new;
         else need = m_new > m_used + kRescaleThreshold;
         if (__ballot_sync(0xffffffffu, need)) {
-          // O is being accumulated by PV(t-1): wait for it (PV(t-2) is known complete, so the parity is unambiguous).
-          // Both warps of a pair take this branch together (same m_new); each rescales half of O's columns.
-          mbar_wait(bar(BAR_PV_DONE), (t - 1) & 1);
+          // O is being accumulated by PV(t-1): wait for it.  PV(t) commits to barrier t&1, so the parity of use
+          // (t-1)/2 of barrier (t-1)&1 is unambiguous.  All threads of a row take this branch together (same m_new);
+          // each rescales its own columns of O.
+          mbar_wait(bar(BAR_PV_DONE + ((t - 1) & 1)), ((t - 1) >> 1) & 1);
           tc_fence_after();
           const float f = need ? ex2_approx(m_used - m_new) : 1.0f;
           if (need) { m_used = m_new; l *= f; }
 #pragma unroll 1
-          for (int c = 0; c < D / 32; ++c) {             // rare path: small chunks keep the register footprint low
+          for (int c = 0; c < QE / 16; ++c) {            // rare path: small chunks keep the register footprint low
             uint32_t o[16];
-            const uint32_t o_addr = tmem + lane_base + kOCol + part * (D / 2) + c * 16;
+            const uint32_t o_addr = tmem + lane_base + kOCol + part * QE + c * 16;
             tmem_ld16(o_addr, o);
             tc_wait_ld();
 #pragma unroll
@@ -321,37 +346,40 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
           unpack2(add2(sum_a, sum_b), a0, a1);
           l += a0 + a1;
         }
-        if constexpr (CW == 32) tmem_st16(s_addr + part * (CW / 2), pk);
-        else tmem_st8(s_addr + part * (CW / 2), pk);
+        tmem_st8(s_addr + part * (CW / 2), pk);
         tc_wait_st();
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(bar(BAR_P_FULL + (t & 1)));
+        if (lane == 0) mbar_arrive(bar(BAR_P_FULL + u));
       }
 
-      // epilogue: O / l -> bf16, stored in linear token order (no untile pass); each thread of a pair stores half a row
-      sXch[(4 + part) * 128 + row] = l;
-      named_bar_sync(1 + sw, 64);
-      l += sXch[(4 + (part ^ 1)) * 128 + row];
+      // epilogue: O / l -> bf16, stored in linear token order (no untile pass); each thread stores its QE columns
+      {
+        const int xb = T % kSBufs;                     // exchange buffer not used by the last half-tile
+        sXch[(xb * NPART + part) * 128 + row] = l;
+        named_bar_sync(1 + sw, NPART * 32);
+        l = 0.f;
+#pragma unroll
+        for (int q = 0; q < NPART; ++q) l += sXch[(xb * NPART + q) * 128 + row];
+      }
       mbar_wait(bar(BAR_O_FULL), 0);
       tc_fence_after();
       const float inv_l = 1.0f / l;
-      const bool live = row < valid_q;
-      uint16_t *orow = p.o + (((int64_t)b * p.H + h) * p.Lq + (int64_t)i * BLK + row) * D + part * (D / 2);
+      uint16_t *orow = p.o + (((int64_t)b * p.H + h) * p.Lq + (int64_t)i * BLK + row) * D + part * QE;
 #pragma unroll
-      for (int c = 0; c < D / 64; ++c) {
-        uint32_t o[32];
-        tmem_ld32(tmem + lane_base + kOCol + part * (D / 2) + c * 32, o);
+      for (int c = 0; c < QE / 16; ++c) {
+        uint32_t o[16];
+        tmem_ld16(tmem + lane_base + kOCol + part * QE + c * 16, o);
         tc_wait_ld();
         if (live) {
 #pragma unroll
-          for (int e = 0; e < 32; e += 8) {
+          for (int e = 0; e < 16; e += 8) {
             uint4 v;
             v.x = pack_bf16x2(__uint_as_float(o[e + 0]) * inv_l, __uint_as_float(o[e + 1]) * inv_l);
             v.y = pack_bf16x2(__uint_as_float(o[e + 2]) * inv_l, __uint_as_float(o[e + 3]) * inv_l);
             v.z = pack_bf16x2(__uint_as_float(o[e + 4]) * inv_l, __uint_as_float(o[e + 5]) * inv_l);
             v.w = pack_bf16x2(__uint_as_float(o[e + 6]) * inv_l, __uint_as_float(o[e + 7]) * inv_l);
-            *reinterpret_cast<uint4 *>(orow + c * 32 + e) = v;
+            *reinterpret_cast<uint4 *>(orow + c * 16 + e) = v;
           }
         }
       }
@@ -372,15 +400,14 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
 
   tc_fence_before();
   __syncthreads();
-  if (warp == kMmaWarp) tmem_dealloc(tmem, kTmemCols);
+  if (warp == L::kMmaWarp) tmem_dealloc(tmem, kTmemCols);
 }
 
 template <int D, int BLK>
-static int launch_one(const AttnParams &ap, const BatchMeta &meta, const CUtensorMap &tm_q, const CUtensorMap &tm_k_full,
-                      const CUtensorMap &tm_k_8, const CUtensorMap &tm_v_full, const CUtensorMap &tm_v_8,
-                      cudaStream_t st) {
+static int launch_one(const AttnParams &ap, const BatchMeta &meta, const CUtensorMap &tm_k_full, const CUtensorMap &tm_k_8,
+                      const CUtensorMap &tm_v_full, const CUtensorMap &tm_v_8, cudaStream_t st) {
   auto kern = li_sparse_attn_kernel<D, BLK>;
-  constexpr int smem = AttnSmem<D, BLK>::kTotal;
+  constexpr int smem = AttnCfg<D, BLK>::kTotal;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   if (e != cudaSuccess) return (int)e;
   cudaLaunchAttribute attr[1];
@@ -388,24 +415,23 @@ static int launch_one(const AttnParams &ap, const BatchMeta &meta, const CUtenso
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(ap.Nqb, ap.H, ap.B);
-  cfg.blockDim = dim3(kThreads);
+  cfg.blockDim = dim3(AttnCfg<D, BLK>::kThreads);
   cfg.dynamicSmemBytes = smem;
   cfg.stream = st;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  e = cudaLaunchKernelEx(&cfg, kern, ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8);
-  if (e != cudaSuccess) return (int)e;
-  return (int)cudaGetLastError();
+  e = cudaLaunchKernelEx(&cfg, kern, ap, meta, tm_k_full, tm_k_8, tm_v_full, tm_v_8);
+  return (int)e;
 }
 
-int launch_attn(const AttnParams &ap, const BatchMeta &meta, int d, int blk, const CUtensorMap &tm_q,
-                const CUtensorMap &tm_k_full, const CUtensorMap &tm_k_8, const CUtensorMap &tm_v_full,
-                const CUtensorMap &tm_v_8, cudaStream_t st, int64_t *n_launches) {
+int launch_attn(const AttnParams &ap, const BatchMeta &meta, int d, int blk, const CUtensorMap &tm_k_full,
+                const CUtensorMap &tm_k_8, const CUtensorMap &tm_v_full, const CUtensorMap &tm_v_8, cudaStream_t st,
+                int64_t *n_launches) {
   int e;
-  if (d == 128 && blk == 128) e = launch_one<128, 128>(ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st);
-  else if (d == 128 && blk == 64) e = launch_one<128, 64>(ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st);
-  else if (d == 64 && blk == 128) e = launch_one<64, 128>(ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st);
-  else e = launch_one<64, 64>(ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st);
+  if (d == 128 && blk == 128) e = launch_one<128, 128>(ap, meta, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st);
+  else if (d == 128 && blk == 64) e = launch_one<128, 64>(ap, meta, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st);
+  else if (d == 64 && blk == 128) e = launch_one<64, 128>(ap, meta, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st);
+  else e = launch_one<64, 64>(ap, meta, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st);
   if (e == 0 && n_launches) *n_launches += 1;
   return e;
 }
