@@ -3,6 +3,8 @@
 // launch counter and the lazily resolved cuTensorMapEncodeTiled entry point.
 #include <atomic>
 #include <cmath>
+#include <cstdio>
+#include <cstdlib>
 #include <cstring>
 
 #include "li_internal.h"
@@ -174,10 +176,15 @@ int li_sparse_attn(const li_problem *p, const int32_t *sel_idx, const int32_t *s
   ap.scale_log2 = scale * 1.4426950408889634f;
   ap.frame_idx = p->frame_idx; ap.sel_idx = sel_idx; ap.sel_cnt = sel_cnt;
   ap.o = (uint16_t *)o; ap.lse = lse_opt;
+#ifdef LI_TRACE
+  ap.trace = (long long *)workspace;      // debug builds: the (otherwise unused) workspace receives the timeline
+#endif
   ap.q = (const uint16_t *)p->q; ap.q_sb = p->q_sb; ap.q_sh = p->q_sh; ap.q_st = p->q_st;
   int64_t n = 0;
   const int e = li::launch_attn(ap, dv.meta, p->d, blk, tm_kf, tm_k8, tm_vf, tm_v8, (cudaStream_t)cuda_stream, &n);
   g_launches += n;
+  if (e != 0 && std::getenv("LI_DEBUG") != nullptr)
+    std::fprintf(stderr, "li_sparse_attn: CUDA error %d: %s\n", e, cudaGetErrorString((cudaError_t)e));
   return e == 0 ? LI_OK : LI_ERR_CUDA;
 }
 

@@ -41,6 +41,7 @@ struct AttnParams {
   const int32_t *sel_cnt;
   uint16_t *o;
   float *lse;
+  long long *trace;       // debug timeline (LI_TRACE builds only), else nullptr
 };
 
 // launches (defined in the .cu files); return cudaError_t as int
