@@ -35,9 +35,9 @@ namespace li {
 constexpr int kSelCap = 1024;       // selected-block indices staged in shared memory (rest read from global)
 constexpr int kPageCap = 512;       // frame-list entries staged in shared memory (rest read from global)
 constexpr int kTmemCols = 512;
-constexpr int kQCol = 0, kSCol = 64, kSStride = 64, kOCol = 256, kOStride = 128;   // two O accumulators
+// TMEM columns: Q | S of group 0, 1 | P of group 0, 1 | O of group 0, 1
+constexpr int kQCol = 0, kSCol = 64, kSStride = 64, kPCol = 192, kPStride = 32, kOCol = 256, kOStride = 128;
 constexpr int kStages = 4;          // slots of the K ring and of the V ring (half-tiles)
-constexpr int kSBufs = 3;
 constexpr float kRescaleThreshold = 8.0f;   // log2 units: P stays <= 2^8 between lazy rescales
 #ifndef LI_EMU_OF_4
 #define LI_EMU_OF_4 0
@@ -46,14 +46,18 @@ constexpr float kRescaleThreshold = 8.0f;   // log2 units: P stays <= 2^8 betwee
 #define LI_EARLY_PREFETCH 0
 #endif
 constexpr bool kEarlyPrefetch = LI_EARLY_PREFETCH != 0;   // prefetch the first half of S(t+2) in the middle of exp(t)
+#ifndef LI_STAGGER
+#define LI_STAGGER 800
+#endif
+constexpr long long kStaggerCycles = LI_STAGGER;          // start offset of softmax group 1 (SM clocks)
 constexpr int kEmuOf4 = LI_EMU_OF_4;        // of every 4 column pairs, how many use the FMA-pipe exp2
 
 template <int D, int BLK>
 struct AttnCfg {
   static constexpr int HALF = BLK / 2;
   static constexpr int kSoftmaxWarps = 8;              // two groups of 4 warps (even / odd half-tiles)
-  static constexpr int kProducerK = kSoftmaxWarps, kProducerV = kSoftmaxWarps + 1, kMmaWarp = kSoftmaxWarps + 2;
-  static constexpr int kThreads = (kSoftmaxWarps + 3) * 32;
+  static constexpr int kProducerK = kSoftmaxWarps, kProducerV = kSoftmaxWarps + 1, kMmaWarp = kSoftmaxWarps + 2;   // + g
+  static constexpr int kThreads = (kSoftmaxWarps + 4) * 32;
   static constexpr int kKVChunk = HALF * 128;          // bytes of one 64-column chunk of a K or V half-tile
   static constexpr int kStage = (D / 64) * kKVChunk;
   static constexpr int kOffRing = 0;
@@ -67,11 +71,13 @@ struct AttnCfg {
 enum {
   BAR_FULL = 0,                        // +ring*kStages + slot   (ring 0 = K, 1 = V)
   BAR_EMPTY = BAR_FULL + 2 * kStages,  // +ring*kStages + slot
-  BAR_S_FULL = BAR_EMPTY + 2 * kStages,  // +buffer
-  BAR_P_FULL = BAR_S_FULL + kSBufs,    // +buffer
-  BAR_PV_DONE = BAR_P_FULL + kSBufs,   // +(t & 1)
-  BAR_Q_READY = BAR_PV_DONE + 2,
-  BAR_O_FULL,
+  BAR_S_FULL = BAR_EMPTY + 2 * kStages,  // +group: S(t) of the group is in tensor memory
+  BAR_S_FREE = BAR_S_FULL + 2,         // +group: the group's softmax warps have S(t) in registers (4 arrivals)
+  BAR_P_FULL = BAR_S_FREE + 2,         // +group: P(t) is in tensor memory (4 arrivals)
+  BAR_PV_DONE = BAR_P_FULL + 2,        // +group: O[g] += P(t) V(t) has completed
+  BAR_Q_READY = BAR_PV_DONE + 2,       // Q is in tensor memory (8 arrivals)
+  BAR_O_FULL,                          // +group: the group's last PV has completed
+  BAR_O_FULL1,
   BAR_COUNT
 };
 
@@ -116,8 +122,8 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
     tma_prefetch_desc(&tm_k_8);
     tma_prefetch_desc(&tm_v_8);
     for (int k = 0; k < BAR_COUNT; ++k) {
-      const bool p_full = k >= BAR_P_FULL && k < BAR_P_FULL + kSBufs;
-      mbar_init(bar(k), p_full ? 4 : (k == BAR_Q_READY ? L::kSoftmaxWarps : 1));
+      const bool by_group = k >= BAR_S_FREE && k < BAR_P_FULL + 2;       // S_FREE[2], P_FULL[2]: one arrival per warp
+      mbar_init(bar(k), by_group ? 4 : (k == BAR_Q_READY ? L::kSoftmaxWarps : 1));
     }
     mbar_fence_init();
     fence_proxy_async();
@@ -206,21 +212,24 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
         }
         __syncwarp();
       }
-    } else if (warp == L::kMmaWarp) {
-      // =============================== MMA issuer ===============================
-      // The whole warp walks the loop converged (barrier waits, descriptor arithmetic on warp-uniform values);
-      // one elected lane issues the tcgen05 instructions.
+    } else if (warp >= L::kMmaWarp) {
+      // =============================== MMA issuers (one warp per softmax group) ===============================
+      // Warp g issues, for its group's half-tiles t = g, g+2, ...:   QK(g) | QK(t+2) PV(t) | QK(t+4) PV(t+2) | ...
+      // i.e. the next S is requested as soon as the softmax warps have pulled the current one into registers
+      // (S_FREE), and O[g] += P(t) V(t) as soon as P(t) is published.  The whole warp walks the loop converged; one
+      // elected lane issues the tcgen05 instructions.
+      const int g = warp - L::kMmaWarp;
       constexpr uint32_t idesc_qk = idesc_bf16(128, HALF, 0);
       constexpr uint32_t idesc_pv = idesc_bf16(128, D, 1);
       auto issue_qk = [&](int t) {                   // S(t) = Q K(t)^T, Q read from tensor memory
-        const int slot = t & (kStages - 1);
+        const int slot = t & (kStages - 1), k = t >> 1;
         const uint32_t sK = sRing + slot * L::kStage;
+        if (k > 0) mbar_wait(bar(BAR_S_FREE + g), (k - 1) & 1);      // S(t-2) has left tensor memory
         mbar_wait(bar(BAR_FULL + slot), (t / kStages) & 1);
-        TR(16, 1, t);
         tc_fence_after();
         if (elect_one()) {
           const uint64_t db0 = smem_desc_sw128(sK, 16, 1024);
-          const uint32_t d_s = tmem + kSCol + (t % kSBufs) * kSStride;
+          const uint32_t d_s = tmem + kSCol + g * kSStride;
 #pragma unroll
           for (int kk = 0; kk < D / 16; ++kk) {
             // descriptor of the kk-th 16-channel slice: start address advances by 32 B inside the 128-B row, by one
@@ -228,39 +237,35 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
             const uint64_t db = db0 + (uint64_t)(((kk >> 2) * L::kKVChunk + (kk & 3) * 32) >> 4);
             mma_ts(d_s, tmem + kQCol + kk * 8, db, idesc_qk, kk > 0);
           }
-          TR(16, 5, t);
           mma_commit(bar(BAR_EMPTY + slot));
-          mma_commit(bar(BAR_S_FULL + (t % kSBufs)));
-          TR(16, 6, t);
+          mma_commit(bar(BAR_S_FULL + g));
         }
         __syncwarp();
       };
-      mbar_wait(bar(BAR_Q_READY), 0);
-      tc_fence_after();
-      for (int t = 0; t < kSBufs && t < T; ++t) issue_qk(t);
-      for (int t = 0; t < T; ++t) {
-        // O[t & 1] += P(t) V(t)
-        const int slot = t & (kStages - 1);
-        const uint32_t sV = sRing + (kStages + slot) * L::kStage;
-        mbar_wait(bar(BAR_FULL + kStages + slot), (t / kStages) & 1);
-        TR(16, 2, t);
-        mbar_wait(bar(BAR_P_FULL + (t % kSBufs)), (t / kSBufs) & 1);
-        TR(16, 3, t);
+      if (g < T) {
+        mbar_wait(bar(BAR_Q_READY), 0);
         tc_fence_after();
-        if (elect_one()) {
-          const uint64_t db0 = smem_desc_sw128(sV, L::kKVChunk, 1024);
-          const uint32_t d_o = tmem + kOCol + (t & 1) * kOStride, a_p = tmem + kSCol + (t % kSBufs) * kSStride;
+        issue_qk(g);
+        for (int t = g; t < T; t += 2) {
+          if (t + 2 < T) issue_qk(t + 2);
+          // O[g] += P(t) V(t)
+          const int slot = t & (kStages - 1), k = t >> 1;
+          const uint32_t sV = sRing + (kStages + slot) * L::kStage;
+          mbar_wait(bar(BAR_FULL + kStages + slot), (t / kStages) & 1);
+          mbar_wait(bar(BAR_P_FULL + g), k & 1);
+          tc_fence_after();
+          if (elect_one()) {
+            const uint64_t db0 = smem_desc_sw128(sV, L::kKVChunk, 1024);
+            const uint32_t d_o = tmem + kOCol + g * kOStride, a_p = tmem + kPCol + g * kPStride;
 #pragma unroll
-          for (int kk = 0; kk < HALF / 16; ++kk)
-            mma_ts(d_o, a_p + kk * 8, db0 + (uint64_t)((kk * 2048) >> 4), idesc_pv, (t > 1 || kk > 0) ? 1u : 0u);
-          TR(16, 7, t);
-          mma_commit(bar(BAR_EMPTY + kStages + slot));
-          mma_commit(bar(BAR_PV_DONE + (t & 1)));
-          if (t == T - 1) mma_commit(bar(BAR_O_FULL));
-          TR(16, 4, t);
+            for (int kk = 0; kk < HALF / 16; ++kk)
+              mma_ts(d_o, a_p + kk * 8, db0 + (uint64_t)((kk * 2048) >> 4), idesc_pv, (k > 0 || kk > 0) ? 1u : 0u);
+            mma_commit(bar(BAR_EMPTY + kStages + slot));
+            mma_commit(bar(BAR_PV_DONE + g));
+            if (t + 2 >= T) mma_commit(bar(BAR_O_FULL + g));
+          }
+          __syncwarp();
         }
-        __syncwarp();
-        if (t + kSBufs < T) issue_qk(t + kSBufs);
       }
     } else {
       // =============================== softmax / lazy correction / epilogue ===============================
@@ -301,11 +306,17 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
       };
       constexpr int NLD = HALF / 32;                             // 32-column TMEM loads per S row
       auto wait_s = [&](int t) {
-        mbar_wait(bar(BAR_S_FULL + t % kSBufs), (t / kSBufs) & 1);
+        mbar_wait(bar(BAR_S_FULL + g), (t >> 1) & 1);
         tc_fence_after();
       };
       auto load_s = [&](int t, int c, uint32_t (&dst)[HALF]) {   // columns [32c, 32c+32) of S(t) -> registers (no wait::ld)
-        tmem_ld32(tmem + lane_base + kSCol + (t % kSBufs) * kSStride + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&dst[c * 32]));
+        tmem_ld32(tmem + lane_base + kSCol + g * kSStride + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&dst[c * 32]));
+      };
+      auto release_s = [&]() {                                   // S is in registers: its TMEM buffer may be overwritten
+        tc_wait_ld();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar(BAR_S_FREE + g));
       };
       // one half-tile: `cur` holds S(t); S(t+2) is prefetched into `nxt` while P(t) is being computed
       auto step = [&](int t, uint32_t (&cur)[HALF]) {
@@ -314,7 +325,7 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
         const int hv = min(HALF, tile_valid(j) - hh * HALF);     // valid key columns of this half-tile (> 0)
         advance();
         if (t + 1 < T) advance();
-        const int u = t % kSBufs;
+        const int k = t >> 1;                            // this is the group's k-th half-tile
         if (hv < HALF) {                                         // padded key columns -> -inf (warp-uniform branch)
 #pragma unroll
           for (int c = 0; c < HALF; ++c) if (c >= hv) cur[c] = 0xff800000u;
@@ -337,7 +348,7 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
         if (__ballot_sync(0xffffffffu, need)) {
           // this group's O is being accumulated by PV(t-2), which commits to PV_DONE[g] as its use number (t-2)/2;
           // PV(t-4) is known complete (S(t) exists), so the parity test is unambiguous
-          mbar_wait(bar(BAR_PV_DONE + g), ((t >> 1) - 1) & 1);
+          mbar_wait(bar(BAR_PV_DONE + g), (k - 1) & 1);
           tc_fence_after();
           const float f = need ? ex2_approx(m_used - m_new) : 1.0f;
           if (need) { m_used = m_new; l *= f; }
@@ -391,18 +402,23 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
           l += a0 + a1;
         }
         TR(warp, 5, t);
-        const uint32_t p_addr = tmem + lane_base + kSCol + u * kSStride;
+        // P(t) goes to the group's own P columns, which PV(t-2) must have finished reading
+        if (k > 0) {
+          mbar_wait(bar(BAR_PV_DONE + g), (k - 1) & 1);
+          tc_fence_after();
+        }
+        const uint32_t p_addr = tmem + lane_base + kPCol + g * kPStride;
         if constexpr (HALF == 64) tmem_st32(p_addr, *reinterpret_cast<uint32_t(*)[32]>(&pk[0]));
         else tmem_st16(p_addr, pk);
         tc_wait_st();
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(bar(BAR_P_FULL + u)); // P(t) is published BEFORE waiting for S(t+2): QK(t+2) may
-        TR(warp, 7, t);                                  // itself be queued behind the other group's PV
+        if (lane == 0) mbar_arrive(bar(BAR_P_FULL + g));
+        TR(warp, 7, t);
         if (more) {
           if (!kEarlyPrefetch) { wait_s(t + 2); load_s(t + 2, 0, nxt); }
           if (NLD == 2) load_s(t + 2, 1, nxt);
-          tc_wait_ld();                                  // S(t+2) row is now in registers
+          release_s();                                   // S(t+2) row is now in registers
         }
         TR(warp, 8, t);
       };
@@ -411,10 +427,17 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
         uint32_t sa[HALF];
         if (g < T) {
           if (g == 1) advance();                         // group 1 starts at half-tile 1
+          if (g == 1 && kStaggerCycles > 0) {
+            // start the second group half a step late: two groups in phase would fight for the MUFU during their
+            // exponentials and leave it idle during their other phases
+            const long long t_start = clock64();
+            while (clock64() - t_start < kStaggerCycles) {
+            }
+          }
           wait_s(g);
 #pragma unroll
           for (int c = 0; c < NLD; ++c) load_s(g, c, sa);
-          tc_wait_ld();
+          release_s();
           for (int t = g; t < T; t += 2) step(t, sa);
         }
       }
@@ -431,6 +454,7 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
       const float wA = (g == 0 ? w_me : w_o) / l_all, wB = (g == 0 ? w_o : w_me) / l_all;
       const bool hasB = T > 1;
       mbar_wait(bar(BAR_O_FULL), 0);
+      if (hasB) mbar_wait(bar(BAR_O_FULL1), 0);
       tc_fence_after();
       uint16_t *orow = p.o + (((int64_t)b * p.H + h) * p.Lq + (int64_t)i * BLK + row) * D + g * QE;
 #pragma unroll
