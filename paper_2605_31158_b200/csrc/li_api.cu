@@ -159,8 +159,9 @@ int li_sparse_attn(const li_problem *p, const int32_t *sel_idx, const int32_t *s
   const int blk = p->block_k;
   const int half = blk / 2;                 // K/V are fetched as half-tiles of blk/2 rows
   const int has_full = p->frame_tokens >= half ? 1 : 0;
-  CUtensorMap tm_kf, tm_k8, tm_vf, tm_v8;
-  bool ok = encode_map(&tm_k8, p->k_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp, 8);
+  CUtensorMap tm_q, tm_kf, tm_k8, tm_vf, tm_v8;
+  bool ok = encode_map(&tm_q, p->q, p->d, p->Lq, p->H, p->B, p->q_st, p->q_sh, p->q_sb, blk);
+  ok = ok && encode_map(&tm_k8, p->k_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp, 8);
   ok = ok && encode_map(&tm_v8, p->v_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp, 8);
   ok = ok && encode_map(&tm_kf, p->k_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp,
                         has_full ? half : 8);
@@ -176,12 +177,8 @@ int li_sparse_attn(const li_problem *p, const int32_t *sel_idx, const int32_t *s
   ap.scale_log2 = scale * 1.4426950408889634f;
   ap.frame_idx = p->frame_idx; ap.sel_idx = sel_idx; ap.sel_cnt = sel_cnt;
   ap.o = (uint16_t *)o; ap.lse = lse_opt;
-#ifdef LI_TRACE
-  ap.trace = (long long *)workspace;      // debug builds: the (otherwise unused) workspace receives the timeline
-#endif
-  ap.q = (const uint16_t *)p->q; ap.q_sb = p->q_sb; ap.q_sh = p->q_sh; ap.q_st = p->q_st;
   int64_t n = 0;
-  const int e = li::launch_attn(ap, dv.meta, p->d, blk, tm_kf, tm_k8, tm_vf, tm_v8, (cudaStream_t)cuda_stream, &n);
+  const int e = li::launch_attn(ap, dv.meta, p->d, blk, tm_q, tm_kf, tm_k8, tm_vf, tm_v8, (cudaStream_t)cuda_stream, &n);
   g_launches += n;
   if (e != 0 && std::getenv("LI_DEBUG") != nullptr)
     std::fprintf(stderr, "li_sparse_attn: CUDA error %d: %s\n", e, cudaGetErrorString((cudaError_t)e));

@@ -34,19 +34,17 @@ struct AttnParams {
   int32_t B, H, Lq, T_f, n_cur, Nqb, Nc, kmax;
   int32_t has_box_full;   // 1: tensor maps with a full-block box exist (T_f >= block)
   float scale_log2;       // softmax_scale * log2(e)
-  const uint16_t *q;      // Q[B,H,Lq,d], read once per CTA straight into tensor memory
-  int64_t q_sb, q_sh, q_st;
   const int32_t *frame_idx;
   const int32_t *sel_idx;
   const int32_t *sel_cnt;
   uint16_t *o;
   float *lse;
-  long long *trace;       // debug timeline (LI_TRACE builds only), else nullptr
 };
 
 // launches (defined in the .cu files); return cudaError_t as int
 int launch_select(const SelectParams &sp, const BatchMeta &meta, cudaStream_t st, int64_t *n_launches);
-int launch_attn(const AttnParams &ap, const BatchMeta &meta, int d, int blk, const CUtensorMap &tm_k_full, const CUtensorMap &tm_k_8, const CUtensorMap &tm_v_full,
+int launch_attn(const AttnParams &ap, const BatchMeta &meta, int d, int blk, const CUtensorMap &tm_q,
+                const CUtensorMap &tm_k_full, const CUtensorMap &tm_k_8, const CUtensorMap &tm_v_full,
                 const CUtensorMap &tm_v_8, cudaStream_t st, int64_t *n_launches);
 
 }  // namespace li
