@@ -157,6 +157,22 @@ def run_reference(args):
     return 0
 
 
+# ------------------------------------------------------------------------------------------ multi-rank plumbing
+def max_over_ranks(values, device, world):
+    """Device-side timings of this rank -> the slowest rank's (the job's) timings.  The path has no exchange step
+    (replicas only), so this all-reduce of a few scalars AFTER the timed region is the only collective."""
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
+def job_throughput(flops_per_replica_step, steps, world, total_ms):
+    """Whole-job TFLOP/s: every rank runs one replica of the workload (weak scaling)."""
+    return world * flops_per_replica_step * steps / (total_ms * 1e-3) / 1e12
+
+
 # ------------------------------------------------------------------------------------------ CUDA arm
 def run_cuda(args):
     import torch.distributed as dist
@@ -267,14 +283,11 @@ def run_cuda(args):
     h2d = q_host.numel() * 2 + fi_host.numel() * 4 + kcur_host.numel() * 2 + vcur_host.numel() * 2
     d2h = o_host.numel() * 2
 
-    t = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms, e2e_ms = float(t[0]), float(t[1])
+    total_ms, e2e_ms = max_over_ranks([total_ms, e2e_ms], dev, world)
     if rank == 0:
         pk = peaks()
-        value = world * flops * args.steps / (total_ms * 1e-3) / 1e12
-        e2e_val = world * flops * args.steps / (e2e_ms * 1e-3) / 1e12
+        value = job_throughput(flops, args.steps, world, total_ms)
+        e2e_val = job_throughput(flops, args.steps, world, e2e_ms)
         attn_tflops = flops / (float(att_ms.mean()) * 1e-3) / 1e12
         sel_bytes = sum((prob.Lq + prob.L_hist(b)) * s.d * 2 * s.H for b in range(prob.B))
         line = {
