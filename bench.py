@@ -33,7 +33,7 @@ METRIC = "sparse-attn effective TFLOP/s over attended blocks (select + attention
 UNIT = "TFLOP/s"
 # dram__bytes_read.sum + dram__bytes_write.sum of li_sparse_attn_kernel<128,128> per launch, from the
 # `ncu --set full` capture summarised in profiles/ (None until that capture exists for this workload).
-NCU_TRAFFIC_BYTES = {"mid": None}
+NCU_TRAFFIC_BYTES = {"mid": 391319040}   # profiles/r1_final_mid_ncu_full_summary.txt: 359.61 MB read + 31.71 MB written
 
 
 def peaks():
@@ -332,7 +332,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--config", default="mid", choices=["tiny", "mid", "long", "adaptive", "dense-equivalence"])
-    ap.add_argument("--ref-heads", type=int, default=2, help="heads in the oracle's bounded sample")
+    ap.add_argument("--ref-heads", type=int, default=24, help="heads in the oracle's bounded sample")
     ap.add_argument("--ref-tiles", type=int, default=None, help="query blocks per head in the oracle's sample (default all)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     args = ap.parse_args()
