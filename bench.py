@@ -308,7 +308,7 @@ def run_cuda(args):
                          "kernel": "li_sparse_attn_kernel", "peak_source": pk["source"] + " burst bf16"},
             "roofline_select": {"bound": "hbm", "achieved": sel_bytes / (float(sel_ms.mean()) * 1e-3) / 1e9, "peak": pk["hbm_gbs"],
                                 "unit": "GB/s", "frac": sel_bytes / (float(sel_ms.mean()) * 1e-3) / 1e9 / pk["hbm_gbs"],
-                                "kernel": "li_pool_kernel + li_score_topk_kernel"},
+                                "kernel": "li_pool_kernel + li_score_kernel + li_topk_kernel"},
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "ms_per_step": e2e_ms / args.steps,
                     "note": "per step: Q, frame list and the chunk's K/V pages copied from pinned host memory, O read back; "
