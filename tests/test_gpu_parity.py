@@ -167,3 +167,63 @@ def test_growing_row_maximum_exercises_lazy_rescale(P):
         prob.k_cache[pg] = (prob.k_cache[pg].float() * (1.0 + 1.5 * rank)).to(torch.bfloat16)
     excused, mx, mean = P.full_parity(prob)
     print(f"small-rescale: excused={excused} max-abs={mx:.3g} mean-abs={mean:.3g}")
+
+
+def test_strided_q_and_token_major_cache(P):
+    """The ABI takes arbitrary (multiple-of-8) strides: Q as a slice of a wider tensor, the cache stored token-major
+    ([page, token, head, d]) and viewed as [page, head, token, d]."""
+    import paper_2605_31158_b200 as li
+    spec = W.spec_small(name="small-strided", H=3, d=128, block=128, frame_tokens=200, n_cur_frames=2, n_pages=10,
+                        n_mem=(2,), n_win=(2,), density=Fraction(1, 2))
+    prob = W.build(spec)
+    dev = "cuda:0"
+    q_wide = torch.zeros((1, spec.H, prob.Lq, 2 * spec.d), dtype=torch.bfloat16, device=dev)
+    q_wide[..., :spec.d] = prob.q.to(dev)
+    q_wide[..., spec.d:] = float("nan")                                      # must never be read
+    q = q_wide[..., :spec.d]
+    kc = prob.k_cache.to(dev).permute(0, 2, 1, 3).contiguous().permute(0, 2, 1, 3)   # same values, token-major memory
+    vc = prob.v_cache.to(dev).permute(0, 2, 1, 3).contiguous().permute(0, 2, 1, 3)
+    assert q.stride(2) == 2 * spec.d and kc.stride(2) == spec.H * spec.d and kc.stride(1) == spec.d
+    ctx = li.Context(q, kc, vc, torch.from_numpy(prob.frame_idx).to(dev), prob.frame_off, spec.n_cur_frames, spec.block)
+    buf = li.Buffers(ctx, prob.kmax, want_scores=True)
+    li.forward(ctx, prob.top_k, buf)
+    torch.cuda.synchronize()
+    osel, osc = P.oracle_select(prob)
+    P.check_selection(prob, buf, osel, osc)
+    o_ref, lse_ref = P.oracle_attn(prob, [g[0] for g in P.gpu_selection(prob, buf)])
+    P.compare_output(buf.o, buf.lse, o_ref, lse_ref)
+
+
+def test_many_blocks_long_lists_and_massive_ties(P):
+    """M = 1200 historical blocks drawn (with repetition) from 6 pages: exact score ties everywhere (lowest index must
+    win), top-k above the register fast path (M > 512), more selected blocks than the kernel stages in shared memory
+    (k = 1100 > 1024) and a frame list longer than its shared-memory copy (1201 > 256)."""
+    import paper_2605_31158_b200 as li
+    from oracle import li_oracle as O
+    g = torch.Generator().manual_seed(11)
+    H, d, T_f, blk, n_hist, k = 1, 64, 64, 64, 1200, 1100
+    q = torch.randn((1, H, T_f, d), generator=g).to(torch.bfloat16)
+    kc = torch.randn((7, H, T_f, d), generator=g).to(torch.bfloat16)
+    vc = torch.randn((7, H, T_f, d), generator=g).to(torch.bfloat16)
+    fi = np.concatenate([torch.randint(0, 6, (n_hist,), generator=g).numpy(), [6]]).astype(np.int32)
+    fo = np.asarray([0, n_hist + 1], np.int32)
+    ctx = li.Context(q.cuda(), kc.cuda(), vc.cuda(), torch.from_numpy(fi).cuda(), fo, 1, blk)
+    buf = li.Buffers(ctx, k, want_scores=True)
+    li.forward(ctx, [k], buf)
+    torch.cuda.synchronize()
+    u16 = lambda t: t.view(torch.int16).numpy().view(np.uint16)
+    osel, osc = O.block_select(u16(q), u16(kc), fi, fo, 1, blk, blk, [k])
+    np.testing.assert_array_equal(buf.sel_idx.cpu().numpy()[0], osel[0])     # ties are exact: bit-identical mask
+    o_ref, lse_ref = O.sparse_attn(u16(q), u16(kc), u16(vc), fi, fo, 1, blk, blk, osel)
+    P.compare_output(buf.o, buf.lse, o_ref, lse_ref)
+
+
+def test_batch_of_64_calls(P):
+    """LI_MAX_CALLS independent calls in one launch, each with its own frame list and top-k."""
+    spec = W.spec_small(name="small-b64", H=1, d=64, block=64, frame_tokens=64, n_cur_frames=1, n_pages=64 * 6,
+                        n_mem=tuple(b % 3 for b in range(64)), n_win=tuple(1 + b % 2 for b in range(64)),
+                        density=Fraction(1, 2), pages_per_call=6)
+    prob = W.build(spec)
+    assert prob.B == 64
+    excused, mx, mean = P.full_parity(prob)
+    print(f"small-b64: excused={excused} max-abs={mx:.3g} mean-abs={mean:.3g}")
