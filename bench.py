@@ -283,6 +283,36 @@ def run_cuda(args):
     h2d = q_host.numel() * 2 + fi_host.numel() * 4 + kcur_host.numel() * 2 + vcur_host.numel() * 2
     d2h = o_host.numel() * 2
 
+    # ---- extras: L2-warm attention, and the cost of the paged gather = attention over the frame-paged
+    #      pool minus attention over the same context laid out contiguously with an identity frame list ----
+    extras = {}
+    if world == 1 and not args.no_extras:
+        def time_attn(cx, n=10, flush_l2=True):
+            ts = []
+            for _ in range(n):
+                if flush_l2:
+                    flush.fill_(3)
+                a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                li.li_sparse_attn(cx, buf.sel_idx, buf.sel_cnt, buf.kmax, buf.o, buf.lse, buf.workspace, stream)
+                b_.record(stream)
+                torch.cuda.synchronize()
+                ts.append(a.elapsed_time(b_))
+            return float(np.mean(ts[2:]))
+        extras["attn_ms_l2_warm"] = time_attn(ctx, flush_l2=False)
+        order = torch.from_numpy(prob.frame_idx.astype(np.int64)).to(dev)
+        free_b = torch.cuda.mem_get_info()[0]
+        need_b = 2 * order.numel() * kc[0].numel() * 2
+        if need_b < free_b // 2:
+            kc2, vc2 = kc.index_select(0, order), vc.index_select(0, order)
+            ident = torch.arange(order.numel(), dtype=torch.int32, device=dev)
+            ctx2 = li.Context(q, kc2, vc2, ident, prob.frame_off, s.n_cur_frames, s.block)
+            t_paged, t_ident = time_attn(ctx), time_attn(ctx2)
+            extras["attn_ms_paged"] = t_paged
+            extras["attn_ms_identity_contiguous"] = t_ident
+            extras["gather_overhead_frac"] = (t_paged - t_ident) / t_ident
+            del kc2, vc2, ctx2
+
     total_ms, e2e_ms = max_over_ranks([total_ms, e2e_ms], dev, world)
     if rank == 0:
         pk = peaks()
@@ -315,6 +345,7 @@ def run_cuda(args):
                             "the historical K/V cache stays resident (it is the cache)"},
             "gpu_launches": int(launches), "clocks": clk.summary(),
         }
+        line.update(extras)
         if not args.no_cpu and world == 1:
             dt, fl, desc = oracle_sample(prob, args.ref_heads, args.ref_tiles)
             line["cpu_baseline"] = {"value": fl / dt / 1e12, "unit": UNIT, "cores": cpu_threads(), "kind": "oracle",
@@ -335,6 +366,7 @@ def main():
     ap.add_argument("--ref-heads", type=int, default=24, help="heads in the oracle's bounded sample")
     ap.add_argument("--ref-tiles", type=int, default=None, help="query blocks per head in the oracle's sample (default all)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-extras", action="store_true", help="skip the L2-warm / gather-overhead measurements")
     args = ap.parse_args()
     if args.impl == "reference":
         if args.steps == 20 and args.warmup == 5:
