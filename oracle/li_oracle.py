@@ -26,8 +26,10 @@ routine) for r=1 and r->0; rows of exp(s-lse) sum to 1; constant V; shift invari
 single attended token; page-permutation / duplicate-page / identity-list invariances; pooled
 means of constant blocks, ragged tails, NaN padding; closed-form ranking; argsort brute
 force; exact ties -> lowest index; k=M; nested selections.
-Nothing in this file is "parity unpinned".  (3-D tiling, text prefix and the policy scalars
-of Eq. 1-8 are not implemented here at all: out of the hot-path scope.)
+The 3-D block tiling of PAPER.md:129/:321 (functions *_3d at the end) is pinned by tests/test_oracle_3d_pins.py:
+explicit coordinate brute force, reduction to the 1-D tiling when blocks are row segments, partition and padding
+properties.  Nothing in this file is "parity unpinned".  (Text prefix and the policy scalars of Eq. 1-8 are not
+implemented here at all: out of the hot-path scope.)
 """
 from __future__ import annotations
 
@@ -193,3 +195,87 @@ def excused_mismatch(scores_row: np.ndarray, k: int, got: Sequence[int], want: S
     if any(m < 0 or m >= len(s) for m in diff):
         return False
     return all(abs(s[m] - kth) <= tol for m in diff)
+
+
+# ============================================================================= 3-D block tiling
+# "tokens are partitioned into non-overlapping 3D blocks of size (B_t, B_h, B_w)"; (4,8,4) on
+# HY-WorldPlay and (4,4,8) on Matrix-Game-3.0, block volume 128 tokens.  A frame is a grid_h x grid_w
+# latent grid in row-major token order (token = y*grid_w + x); a region (history or chunk) of n frames in logical
+# order is tiled by temporal groups of B_t consecutive frames x B_h rows x B_w columns.  Blocks at the bottom / right
+# border and the last temporal group may be partial: "Boundary cases are handled by masked loads",
+# "discarding invalid boundary-padding positions through masked stores" -- i.e. padding never counts.
+# Block order (reading c17): m = (tg * Hb + hb) * Wb + wb, temporal group slowest.
+def blocks_3d(n_frames: int, grid_h: int, grid_w: int, bt: int, bh: int, bw: int) -> List[np.ndarray]:
+    """Logical token indices (frame*T_f + y*grid_w + x, ascending) of every 3-D block of a region of n_frames."""
+    T_f = grid_h * grid_w
+    out = []
+    for tg in range(-(-n_frames // bt)):
+        for hb in range(-(-grid_h // bh)):
+            for wb in range(-(-grid_w // bw)):
+                idx = [f * T_f + y * grid_w + x
+                       for f in range(tg * bt, min(n_frames, (tg + 1) * bt))
+                       for y in range(hb * bh, min(grid_h, (hb + 1) * bh))
+                       for x in range(wb * bw, min(grid_w, (wb + 1) * bw))]
+                out.append(np.asarray(idx, dtype=np.int64))
+    return out
+
+
+def means_over(x: np.ndarray, blocks: Sequence[np.ndarray]) -> np.ndarray:
+    """Eq. 9 over arbitrary token sets: mean of the block's valid tokens, fp64 -> fp32."""
+    out = np.zeros((len(blocks), x.shape[1]), dtype=np.float32)
+    for i, idx in enumerate(blocks):
+        out[i] = x[idx].mean(axis=0).astype(np.float32)
+    return out
+
+
+def block_select_3d(q, k_cache, frame_idx, frame_off, n_cur_frames: int, grid_h: int, grid_w: int, bt: int, bh: int,
+                    bw: int, top_k: Sequence[int]):
+    """li_block_select with 3-D blocks: same steps as block_select, only the token sets of the blocks differ."""
+    B, H, Lq, d = q.shape
+    qblocks = blocks_3d(n_cur_frames if n_cur_frames > 0 else Lq // (grid_h * grid_w), grid_h, grid_w, bt, bh, bw)
+    sel, sc = [], []
+    for b in range(B):
+        hist, _cur = split_frames(frame_idx[frame_off[b]:frame_off[b + 1]], n_cur_frames)
+        kblocks = blocks_3d(len(hist), grid_h, grid_w, bt, bh, bw)
+        idx_b, sc_b = [], []
+        for h in range(H):
+            qbar = means_over(widen(q[b, h]), qblocks)
+            kbar = means_over(gather_logical(k_cache, hist, h), kblocks) if kblocks else np.zeros((0, d), np.float32)
+            s = block_scores(qbar, kbar, d)
+            idx_b.append(top_k_rows(s, min(int(top_k[b]), len(kblocks))))
+            sc_b.append(s)
+        sel.append(np.stack(idx_b))
+        sc.append(np.stack(sc_b))
+    return sel, sc
+
+
+def sparse_attn_3d(q, k_cache, v_cache, frame_idx, frame_off, n_cur_frames: int, grid_h: int, grid_w: int, bt: int,
+                   bh: int, bw: int, sel_idx: Sequence[np.ndarray], softmax_scale: float = 0.0,
+                   tiles: Optional[Sequence[Tuple[int, int, int]]] = None):
+    """li_sparse_attn with 3-D blocks: the queries of 3-D query block i attend ALL chunk tokens plus the valid tokens
+    of the selected 3-D history blocks; outputs in the original linear token order."""
+    B, H, Lq, d = q.shape
+    scale = softmax_scale if softmax_scale != 0.0 else 1.0 / math.sqrt(d)
+    fill = np.nan if tiles is not None else 0.0
+    o = np.full((B, H, Lq, d), fill, dtype=np.float32)
+    lse = np.full((B, H, Lq), fill, dtype=np.float32)
+    qblocks = blocks_3d(n_cur_frames if n_cur_frames > 0 else Lq // (grid_h * grid_w), grid_h, grid_w, bt, bh, bw)
+    todo = tiles if tiles is not None else [(b, h, i) for b in range(B) for h in range(H) for i in range(len(qblocks))]
+    cache = {}
+    for (b, h, i) in todo:
+        if (b, h) not in cache:
+            cache.clear()
+            hist, cur = split_frames(frame_idx[frame_off[b]:frame_off[b + 1]], n_cur_frames)
+            cache[(b, h)] = (gather_logical(k_cache, hist, h), gather_logical(v_cache, hist, h),
+                             gather_logical(k_cache, cur, h), gather_logical(v_cache, cur, h),
+                             blocks_3d(len(hist), grid_h, grid_w, bt, bh, bw))
+        Kh, Vh, Kc, Vc, kblocks = cache[(b, h)]
+        rows = [int(m) for m in np.asarray(sel_idx[b])[h, i] if int(m) >= 0]
+        t = np.concatenate([kblocks[m] for m in rows]) if rows else np.zeros((0,), dtype=np.int64)
+        K = np.concatenate([Kc, Kh[t]], axis=0)
+        V = np.concatenate([Vc, Vh[t]], axis=0)
+        u = qblocks[i]
+        oi, li = softmax_attend(widen(q[b, h])[u], K, V, scale)
+        o[b, h, u] = oi.astype(np.float32)
+        lse[b, h, u] = li.astype(np.float32)
+    return o, lse
