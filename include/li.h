@@ -21,7 +21,8 @@
  *   - Logical order of one call's context: history token t in [0, L_hist) is row t mod T_f of
  *     page F[t div T_f]; chunk token u in [0, Lq) is row u mod T_f of page F[n_hist + u div T_f].
  *     History, chunk and queries are tiled separately from their own first token into blocks of
- *     block_k / block_k / block_q tokens; only the last block of each grid may be partial.
+ *     block_k / block_k / block_q tokens; only the last block of each grid may be partial.  (3-D blocks: see the
+ *     grid_h/grid_w/bt/bh/bw fields of li_problem.)
  *   - There is no CPU fallback and no second backend: without a CUDA device every compute call fails
  *     with LI_ERR_CUDA.
  */
@@ -60,6 +61,16 @@ typedef struct li_problem {
   const int32_t *frame_off_host;/* HOST int32 [B+1]: call b owns frame_idx[frame_off[b] .. frame_off[b+1]) */
   int32_t n_cur_frames;         /* the last n_cur_frames entries of every list are the current chunk (>= 0) */
   float   softmax_scale;        /* 0 => 1/sqrt(d) */
+  /* 3-D block tiling ("non-overlapping 3D blocks of size (B_t,B_h,B_w)", :321 (4,8,4)/(4,4,8), volume
+   * 128).  All five zero = 1-D blocks of block_k consecutive logical tokens.  Otherwise a frame is a grid_h x grid_w
+   * row-major grid (frame_tokens == grid_h*grid_w, token = y*grid_w + x) and a region of n frames (history, chunk,
+   * queries) is tiled by groups of bt consecutive frames x bh rows x bw columns; block index
+   * m = (tg*ceil(grid_h/bh) + hb)*ceil(grid_w/bw) + wb.  Border blocks (grid_h % bh != 0) and the last temporal group
+   * may be partial: padding never enters a mean nor the softmax, and is never stored.
+   * Supported: bt*bh*bw == block_q == block_k, bh*bw == 32, grid_w % bw == 0, Q contiguous over (B,H)
+   * (q_sb == H*q_sh). */
+  int32_t grid_h, grid_w;
+  int32_t bt, bh, bw;
 } li_problem;
 
 /* Eq. 9-10.  For every call b, head h and query block i: pooled means (true cardinality

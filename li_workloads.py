@@ -42,6 +42,8 @@ class Spec:
     k_frame_offset_std: float = 0.0      # `long`: per-(page, head) K mean offsets ~ N(0, std^2)
     pages_per_call: Optional[int] = None # adaptive: call b owns pages [b*ppc, (b+1)*ppc)
     explicit_frames: Optional[List[List[int]]] = None  # tiny: frame list given verbatim
+    grid: Optional[tuple] = None          # (grid_h, grid_w) of a frame, frame_tokens == grid_h*grid_w   } 3-D blocks,
+    block3d: Optional[tuple] = None       # (B_t, B_h, B_w), B_t*B_h*B_w == block                        } PAPER.md:129/:321
 
 
 @dataclasses.dataclass
@@ -69,16 +71,36 @@ class Problem:
     def L_hist(self, b: int) -> int:
         return self.n_hist_frames(b) * self.spec.frame_tokens
 
+    def n_blocks(self, n_frames: int) -> int:
+        """Blocks of a region of n_frames frames (integer bookkeeping of the tiling)."""
+        s = self.spec
+        if s.block3d is not None:
+            (gh, gw), (bt, bh, bw) = s.grid, s.block3d
+            return -(-n_frames // bt) * (-(-gh // bh)) * (-(-gw // bw))
+        return -(-(n_frames * s.frame_tokens) // s.block)
+
+    def block_sizes(self, n_frames: int) -> np.ndarray:
+        """Valid (non-padding) tokens of every block of a region of n_frames frames."""
+        s = self.spec
+        if s.block3d is not None:
+            (gh, gw), (bt, bh, bw) = s.grid, s.block3d
+            ft = [min(bt, n_frames - t * bt) for t in range(-(-n_frames // bt))]
+            fh = [min(bh, gh - y * bh) for y in range(-(-gh // bh))]
+            fw = [min(bw, gw - x * bw) for x in range(-(-gw // bw))]
+            return np.asarray([a * b_ * c for a in ft for b_ in fh for c in fw], dtype=np.int64)
+        L = n_frames * s.frame_tokens
+        return np.asarray([min(s.block, L - m * s.block) for m in range(-(-L // s.block))], dtype=np.int64)
+
     def M(self, b: int) -> int:
-        return -(-self.L_hist(b) // self.spec.block)
+        return self.n_blocks(self.n_hist_frames(b))
 
     @property
     def Nqb(self) -> int:
-        return -(-self.Lq // self.spec.block)
+        return self.n_blocks(self.spec.n_cur_frames)
 
     @property
     def Nc(self) -> int:
-        return -(-(self.spec.n_cur_frames * self.spec.frame_tokens) // self.spec.block)
+        return self.n_blocks(self.spec.n_cur_frames)
 
     @property
     def kmax(self) -> int:
@@ -145,10 +167,11 @@ def build(spec: Spec) -> Problem:
 
     top_k = np.zeros(B, dtype=np.int32)
     for b in range(B):
-        n_hist = len(frames[b]) - spec.n_cur_frames
-        M = -(-(n_hist * T_f) // spec.block)
-        top_k[b] = top_k_for(spec, M)
-    return Problem(spec, q, k_cache, v_cache, frame_idx, frame_off, top_k)
+        top_k[b] = 0
+    prob = Problem(spec, q, k_cache, v_cache, frame_idx, frame_off, top_k)
+    for b in range(B):
+        top_k[b] = top_k_for(spec, prob.M(b))
+    return prob
 
 
 # --------------------------------------------------------------------------------------
@@ -180,9 +203,15 @@ def spec_dense_equivalence(H: int = 24) -> Spec:
                 n_pages=64, n_mem=[4], n_win=[8], density=Fraction(1, 1))
 
 
+def spec_mid3d(H: int = 24) -> Spec:
+    """`mid` with the paper's own block geometry: 30 x 52 latent grid, 3-D blocks (4,8,4)."""
+    return Spec("mid3d", 6006, H=H, d=128, frame_tokens=1560, n_cur_frames=4, block=128, n_pages=64,
+                n_mem=[4], n_win=[8], density=Fraction(1, 4), grid=(30, 52), block3d=(4, 8, 4))
+
+
 def spec_by_name(name: str, H: Optional[int] = None) -> Spec:
     table = {"tiny": spec_tiny, "mid": spec_mid, "long": spec_long, "adaptive": spec_adaptive,
-             "dense-equivalence": spec_dense_equivalence}
+             "dense-equivalence": spec_dense_equivalence, "mid3d": spec_mid3d}
     fn = table[name]
     if name == "tiny" or H is None:
         return fn()
@@ -195,34 +224,26 @@ def spec_by_name(name: str, H: Optional[int] = None) -> Spec:
 def spec_small(name: str = "small", seed: int = 7007, H: int = 2, d: int = 128, block: int = 128,
                frame_tokens: int = 200, n_cur_frames: int = 3, n_pages: int = 12,
                n_mem=(2,), n_win=(3,), density=Fraction(1, 2), top_k=None,
-               k_frame_offset_std: float = 0.0, pages_per_call=None) -> Spec:
+               k_frame_offset_std: float = 0.0, pages_per_call=None, grid=None, block3d=None) -> Spec:
     return Spec(name, seed, H=H, d=d, frame_tokens=frame_tokens, n_cur_frames=n_cur_frames,
                 block=block, n_pages=n_pages, n_mem=list(n_mem), n_win=list(n_win),
                 density=None if top_k is not None else density, top_k=top_k,
-                k_frame_offset_std=k_frame_offset_std, pages_per_call=pages_per_call)
+                k_frame_offset_std=k_frame_offset_std, pages_per_call=pages_per_call, grid=grid, block3d=block3d)
 
 
 def effective_flops(prob: Problem, sel_idx_per_call, sel_cnt_per_call) -> int:
     """4*d*sum_{b,h,i} valid_q(i) * (Lc + sum_{m in I_i} valid_k(m)).
     Pure integer bookkeeping over an ALREADY COMPUTED mask; no method arithmetic."""
     s = prob.spec
-    Bk = s.block
-    Lq = prob.Lq
     Lc = s.n_cur_frames * s.frame_tokens
+    vq = prob.block_sizes(s.n_cur_frames)                      # [Nqb]
     total = 0
     for b in range(prob.B):
-        Lh, M = prob.L_hist(b), prob.M(b)
-        tail = Lh - (M - 1) * Bk if M > 0 else 0
-        idx = np.asarray(sel_idx_per_call[b])          # [H, Nqb, >=k]
-        cnt = np.asarray(sel_cnt_per_call[b])          # [H, Nqb]
-        for i in range(prob.Nqb):
-            vq = min(Bk, Lq - i * Bk)
-            c = cnt[:, i]
-            n_tail = 0
-            if M > 0:
-                kk = idx.shape[-1]
-                mask = (np.arange(kk)[None, :] < c[:, None]) & (idx[:, i, :] == M - 1)
-                n_tail = int(mask.sum())
-            kv = int(c.sum()) * Bk - n_tail * (Bk - tail) + s.H * Lc
-            total += 4 * s.d * vq * kv
+        vk = prob.block_sizes(prob.n_hist_frames(b))           # [M_b]
+        idx = np.asarray(sel_idx_per_call[b])                  # [H, Nqb, >=k]
+        cnt = np.asarray(sel_cnt_per_call[b])                  # [H, Nqb]
+        kk = idx.shape[-1]
+        live = np.arange(kk)[None, None, :] < cnt[:, :, None]
+        tok = np.where(live, vk[np.clip(idx, 0, max(len(vk) - 1, 0))] if len(vk) else 0, 0).sum(axis=-1)   # [H, Nqb]
+        total += int((4 * s.d * vq[None, :] * (tok + Lc)).sum())
     return total

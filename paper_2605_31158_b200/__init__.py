@@ -40,6 +40,8 @@ class li_problem(ctypes.Structure):
         ("kv_sp", ctypes.c_int64), ("kv_sh", ctypes.c_int64), ("kv_st", ctypes.c_int64),
         ("frame_idx", ctypes.c_void_p), ("frame_off_host", ctypes.c_void_p),
         ("n_cur_frames", ctypes.c_int32), ("softmax_scale", ctypes.c_float),
+        ("grid_h", ctypes.c_int32), ("grid_w", ctypes.c_int32),
+        ("bt", ctypes.c_int32), ("bh", ctypes.c_int32), ("bw", ctypes.c_int32),
     ]
 
 
@@ -93,7 +95,8 @@ class Context:
     """Holds one li_problem plus the host arrays it points to (kept alive for the lifetime of the object)."""
 
     def __init__(self, q: torch.Tensor, k_cache: torch.Tensor, v_cache: torch.Tensor, frame_idx: torch.Tensor,
-                 frame_off: Sequence[int], n_cur_frames: int, block: int, softmax_scale: float = 0.0):
+                 frame_off: Sequence[int], n_cur_frames: int, block: int, softmax_scale: float = 0.0,
+                 grid: Optional[Tuple[int, int]] = None, block3d: Optional[Tuple[int, int, int]] = None):
         for t, name in ((q, "q"), (k_cache, "k_cache"), (v_cache, "v_cache")):
             if t.dtype != torch.bfloat16 or not t.is_cuda or t.dim() != 4 or t.stride(-1) != 1:
                 raise ValueError(f"{name} must be a 4-D CUDA bf16 tensor with unit innermost stride")
@@ -121,9 +124,15 @@ class Context:
         p.softmax_scale = softmax_scale
         self.p = p
         self.B, self.H, self.Lq, self.d, self.block = B, H, Lq, d, block
-        self.Nqb = -(-Lq // block)
         n_hist = (self.frame_off[1:] - self.frame_off[:-1]) - n_cur_frames
-        self.M = [-(-(int(n) * p.frame_tokens) // block) for n in n_hist]
+        if block3d is not None:
+            (p.grid_h, p.grid_w), (p.bt, p.bh, p.bw) = grid, block3d
+            per_group = (-(-p.grid_h // p.bh)) * (-(-p.grid_w // p.bw))
+            self.Nqb = -(-(Lq // p.frame_tokens) // p.bt) * per_group
+            self.M = [-(-int(n) // p.bt) * per_group for n in n_hist]
+        else:
+            self.Nqb = -(-Lq // block)
+            self.M = [-(-(int(n) * p.frame_tokens) // block) for n in n_hist]
         self.Mmax = max(self.M) if self.M else 0
 
     def workspace_bytes(self, kmax: int) -> int:

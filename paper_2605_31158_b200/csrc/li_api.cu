@@ -51,6 +51,7 @@ inline size_t mpad(int m) { return m > 0 ? (size_t)((m + 31) & ~31) : 32; }   //
 
 struct Derived {
   int Nqb, Nc, Mmax;
+  li::Tiling tl;
   li::BatchMeta meta;
 };
 
@@ -74,6 +75,17 @@ int check_problem(const li_problem *p, Derived *dv) {
   if (p->q_st < p->d || p->kv_st < p->d) return LI_ERR_INVALID_ARG;
   if (((uintptr_t)p->q | (uintptr_t)p->k_cache | (uintptr_t)p->v_cache) & 15u) return LI_ERR_INVALID_ARG;
   std::memset(&dv->meta, 0, sizeof(dv->meta));
+  std::memset(&dv->tl, 0, sizeof(dv->tl));
+  const bool any3d = p->grid_h | p->grid_w | p->bt | p->bh | p->bw;
+  if (any3d) {
+    if (p->grid_h <= 0 || p->grid_w <= 0 || p->bt <= 0 || p->bh <= 0 || p->bw <= 0) return LI_ERR_INVALID_ARG;
+    if (p->grid_h * p->grid_w != p->frame_tokens) return LI_ERR_INVALID_ARG;
+    if (p->Lq % p->frame_tokens != 0) return LI_ERR_INVALID_ARG;
+    if (p->bt * p->bh * p->bw != p->block_k || p->bh * p->bw != 32 || p->grid_w % p->bw != 0) return LI_ERR_UNSUPPORTED;
+    if (p->q_sb != (int64_t)p->H * p->q_sh && p->B > 1) return LI_ERR_UNSUPPORTED;
+    dv->tl.gh = p->grid_h; dv->tl.gw = p->grid_w; dv->tl.bt = p->bt; dv->tl.bh = p->bh; dv->tl.bw = p->bw;
+    dv->tl.Hb = (p->grid_h + p->bh - 1) / p->bh; dv->tl.Wb = p->grid_w / p->bw;
+  }
   int mmax = 0;
   if (p->frame_off_host[0] < 0) return LI_ERR_INVALID_ARG;
   for (int b = 0; b < p->B; ++b) {
@@ -81,12 +93,13 @@ int check_problem(const li_problem *p, Derived *dv) {
     if (n < p->n_cur_frames) return LI_ERR_INVALID_ARG;
     const int64_t L_hist = (int64_t)(n - p->n_cur_frames) * p->frame_tokens;
     if (L_hist + p->Lq > (int64_t)1 << 30) return LI_ERR_INVALID_ARG;
-    const int M = (int)((L_hist + p->block_k - 1) / p->block_k);
+    const int M = dv->tl.num_blocks(n - p->n_cur_frames, p->frame_tokens, p->block_k);
     if (M > mmax) mmax = M;
   }
   for (int b = 0; b <= p->B; ++b) dv->meta.frame_off[b] = p->frame_off_host[b];
-  dv->Nqb = (p->Lq + p->block_q - 1) / p->block_q;
-  dv->Nc = (p->n_cur_frames * p->frame_tokens + p->block_k - 1) / p->block_k;
+  dv->Nqb = any3d ? dv->tl.num_blocks(p->Lq / p->frame_tokens, p->frame_tokens, p->block_q)
+                  : (p->Lq + p->block_q - 1) / p->block_q;
+  dv->Nc = dv->tl.num_blocks(p->n_cur_frames, p->frame_tokens, p->block_k);
   dv->Mmax = mmax;
   return LI_OK;
 }
@@ -121,7 +134,7 @@ int li_block_select(const li_problem *p, const int32_t *top_k_host, int32_t kmax
   for (int b = 0; b < p->B; ++b) {
     if (top_k_host[b] < 0) return LI_ERR_INVALID_ARG;
     const int n_hist = dv.meta.frame_off[b + 1] - dv.meta.frame_off[b] - p->n_cur_frames;
-    const int M = (int)(((int64_t)n_hist * p->frame_tokens + p->block_k - 1) / p->block_k);
+    const int M = dv.tl.num_blocks(n_hist, p->frame_tokens, p->block_k);
     const int k = top_k_host[b] < M ? top_k_host[b] : M;
     if (k > kmax) return LI_ERR_INVALID_ARG;
     dv.meta.top_k[b] = k;
@@ -129,6 +142,7 @@ int li_block_select(const li_problem *p, const int32_t *top_k_host, int32_t kmax
 
   li::SelectParams sp;
   std::memset(&sp, 0, sizeof(sp));
+  sp.tl = dv.tl;
   sp.B = p->B; sp.H = p->H; sp.Lq = p->Lq; sp.d = p->d; sp.T_f = p->frame_tokens; sp.blk = p->block_k;
   sp.n_cur = p->n_cur_frames; sp.Nqb = dv.Nqb; sp.Mmax = dv.Mmax; sp.kmax = kmax;
   sp.score_pitch = score_pitch;
@@ -171,6 +185,7 @@ int li_sparse_attn(const li_problem *p, const int32_t *sel_idx, const int32_t *s
 
   li::AttnParams ap;
   std::memset(&ap, 0, sizeof(ap));
+  ap.tl = dv.tl;
   ap.B = p->B; ap.H = p->H; ap.Lq = p->Lq; ap.T_f = p->frame_tokens; ap.n_cur = p->n_cur_frames;
   ap.Nqb = dv.Nqb; ap.Nc = dv.Nc; ap.kmax = kmax; ap.has_box_full = has_full;
   const float scale = p->softmax_scale != 0.f ? p->softmax_scale : 1.0f / std::sqrt((float)p->d);

@@ -14,7 +14,18 @@ struct BatchMeta {
   int32_t top_k[LI_MAX_CALLS];          // k_b already clamped to M_b (select only)
 };
 
+// Block tiling of a region of n frames.  bt == 0: 1-D blocks of `blk` consecutive logical tokens.  Otherwise 3-D blocks
+// of bt frames x bh rows x bw columns of the gh x gw frame grid, block index
+// m = (tg*Hb + hb)*Wb + wb; a block's rows are ordered (frame, y, x), 32 = bh*bw rows per frame slice.
+struct Tiling {
+  int32_t gh, gw, bt, bh, bw, Hb, Wb;
+  __host__ __device__ int num_blocks(int n_frames, int T_f, int blk) const {
+    return bt > 0 ? ((n_frames + bt - 1) / bt) * Hb * Wb : (n_frames * T_f + blk - 1) / blk;
+  }
+};
+
 struct SelectParams {
+  Tiling tl;
   int32_t B, H, Lq, d, T_f, blk, n_cur, Nqb, Mmax, Mp, kmax, score_pitch;   // Mp = Mmax rounded up to 32
   const uint16_t *q;
   int64_t q_sb, q_sh, q_st;
@@ -31,6 +42,7 @@ struct SelectParams {
 };
 
 struct AttnParams {
+  Tiling tl;
   int32_t B, H, Lq, T_f, n_cur, Nqb, Nc, kmax;
   int32_t has_box_full;   // 1: tensor maps with a full-block box exist (T_f >= block)
   float scale_log2;       // softmax_scale * log2(e)

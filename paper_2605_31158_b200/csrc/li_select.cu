@@ -35,7 +35,7 @@ __device__ __forceinline__ void add_bf16x8(float (&acc)[8], const uint4 &v) {
 constexpr int kPoolThreads = 256;
 
 // grid = (Nqb + Mmax, H, B).  blockIdx.x < Nqb: query block; otherwise historical K block m = x - Nqb.
-template <int D>
+template <int D, bool K3D>
 __global__ void __launch_bounds__(kPoolThreads) li_pool_kernel(const SelectParams p, const BatchMeta meta) {
   constexpr int TPR = D / 8;                 // threads per row (16-byte loads)
   constexpr int RPP = kPoolThreads / TPR;    // rows per pass
@@ -49,16 +49,45 @@ __global__ void __launch_bounds__(kPoolThreads) li_pool_kernel(const SelectParam
   float *out;
   int out_stride = 1;
 
+  const Tiling tl = p.tl;
+  // 3-D blocks: row r of block m = (tg, hb, wb) is frame tg*bt + r/32, grid row hb*bh + (r%32)/bw,
+  // grid column wb*bw + (r%32)%bw; rows outside the grid or past the region's last frame are padding (not loaded,
+  // not counted: "masked loads").  Returns the token's row inside its frame, or -1 for padding.
+  auto row3d = [&](int m, int r, int n_reg, int &f) -> int {
+    const int per = tl.Hb * tl.Wb, tg = m / per, rem = m - tg * per, hb = rem / tl.Wb, wb = rem - hb * tl.Wb;
+    const int within = r & 31, hh = within / tl.bw, ww = within - hh * tl.bw;
+    f = tg * tl.bt + (r >> 5);
+    const int y = hb * tl.bh + hh;
+    return (f < n_reg && y < tl.gh) ? y * tl.gw + wb * tl.bw + ww : -1;
+  };
+  auto count3d = [&](int m, int n_reg) -> int {
+    const int per = tl.Hb * tl.Wb, tg = m / per, hb = (m - tg * per) / tl.Wb;
+    return min(tl.bt, n_reg - tg * tl.bt) * min(tl.bh, tl.gh - hb * tl.bh) * tl.bw;
+  };
+
   if ((int)blockIdx.x < p.Nqb) {
     const int i = blockIdx.x;
-    const int t0 = i * p.blk;
-    nvalid = min(p.blk, p.Lq - t0);
-    const uint16_t *base = p.q + b * p.q_sb + h * p.q_sh + (int64_t)t0 * p.q_st + cofs;
     uint4 v[kMaxIter];
+    if constexpr (K3D) {
+      const int n_reg = p.Lq / p.T_f;
+      nvalid = count3d(i, n_reg);
+      const uint16_t *base = p.q + b * p.q_sb + h * p.q_sh + cofs;
 #pragma unroll
-    for (int it = 0; it < kMaxIter; ++it) {
-      const int r = r0 + it * RPP;
-      v[it] = r < nvalid ? ldg_stream(base + (int64_t)r * p.q_st) : make_uint4(0, 0, 0, 0);
+      for (int it = 0; it < kMaxIter; ++it) {
+        const int r = r0 + it * RPP;
+        int f;
+        const int row = r < p.blk ? row3d(i, r, n_reg, f) : -1;
+        v[it] = row >= 0 ? ldg_stream(base + ((int64_t)f * p.T_f + row) * p.q_st) : make_uint4(0, 0, 0, 0);
+      }
+    } else {
+      const int t0 = i * p.blk;
+      nvalid = min(p.blk, p.Lq - t0);
+      const uint16_t *base = p.q + b * p.q_sb + h * p.q_sh + (int64_t)t0 * p.q_st + cofs;
+#pragma unroll
+      for (int it = 0; it < kMaxIter; ++it) {
+        const int r = r0 + it * RPP;
+        v[it] = r < nvalid ? ldg_stream(base + (int64_t)r * p.q_st) : make_uint4(0, 0, 0, 0);
+      }
     }
 #pragma unroll
     for (int it = 0; it < kMaxIter; ++it) add_bf16x8(acc, v[it]);
@@ -67,23 +96,35 @@ __global__ void __launch_bounds__(kPoolThreads) li_pool_kernel(const SelectParam
     const int m = blockIdx.x - p.Nqb;
     const int foff = meta.frame_off[b];
     const int n_hist = meta.frame_off[b + 1] - foff - p.n_cur;
-    const int L_hist = n_hist * p.T_f;
-    const int t0 = m * p.blk;
-    if (t0 >= L_hist) return;                // m >= M_b (whole CTA exits together)
-    nvalid = min(p.blk, L_hist - t0);
+    if (m >= tl.num_blocks(n_hist, p.T_f, p.blk)) return;          // m >= M_b (whole CTA exits together)
     const uint16_t *base = p.k_cache + h * p.kv_sh + cofs;
     const int32_t *pages = p.frame_idx + foff;
     uint4 v[kMaxIter];
+    if constexpr (K3D) {
+      nvalid = count3d(m, n_hist);
 #pragma unroll
-    for (int it = 0; it < kMaxIter; ++it) {
-      const int r = r0 + it * RPP;
-      v[it] = make_uint4(0, 0, 0, 0);
-      if (r < nvalid) {
-        const int t = t0 + r;
-        const int pg = t / p.T_f;
-        const int row = t - pg * p.T_f;
-        const int page = __ldg(pages + pg);
-        v[it] = ldg_stream(base + page * p.kv_sp + row * p.kv_st);
+      for (int it = 0; it < kMaxIter; ++it) {
+        const int r = r0 + it * RPP;
+        int f;
+        const int row = r < p.blk ? row3d(m, r, n_hist, f) : -1;
+        v[it] = make_uint4(0, 0, 0, 0);
+        if (row >= 0) v[it] = ldg_stream(base + __ldg(pages + f) * p.kv_sp + row * p.kv_st);
+      }
+    } else {
+      const int L_hist = n_hist * p.T_f;
+      const int t0 = m * p.blk;
+      nvalid = min(p.blk, L_hist - t0);
+#pragma unroll
+      for (int it = 0; it < kMaxIter; ++it) {
+        const int r = r0 + it * RPP;
+        v[it] = make_uint4(0, 0, 0, 0);
+        if (r < nvalid) {
+          const int t = t0 + r;
+          const int pg = t / p.T_f;
+          const int row = t - pg * p.T_f;
+          const int page = __ldg(pages + pg);
+          v[it] = ldg_stream(base + page * p.kv_sp + row * p.kv_st);
+        }
       }
     }
 #pragma unroll
@@ -123,7 +164,7 @@ __global__ void __launch_bounds__(32) li_score_kernel(const SelectParams p, cons
   const int bh = blockIdx.z, b = bh / p.H;
   const int i0 = blockIdx.y * kRowsPerWarp;
   const int n_hist = meta.frame_off[b + 1] - meta.frame_off[b] - p.n_cur;
-  const int M = (n_hist * p.T_f + p.blk - 1) / p.blk;
+  const int M = p.tl.num_blocks(n_hist, p.T_f, p.blk);
   const int m = blockIdx.x * 32 + lane;
   if ((int)blockIdx.x * 32 >= M) return;
   pdl_launch_dependents();
@@ -193,7 +234,7 @@ __global__ void __launch_bounds__(kTopkWarps * 32) li_topk_kernel(const SelectPa
   pdl_wait();                                              // keys come from li_score_kernel
   const int b = (int)(row / ((int64_t)p.H * p.Nqb));
   const int n_hist = meta.frame_off[b + 1] - meta.frame_off[b] - p.n_cur;
-  const int M = (n_hist * p.T_f + p.blk - 1) / p.blk;
+  const int M = p.tl.num_blocks(n_hist, p.T_f, p.blk);
   const int k = min(meta.top_k[b], M);
   const uint32_t *key = p.keys + row * p.Mmax;
   int32_t *out = p.sel_idx + row * p.kmax;
@@ -266,8 +307,13 @@ __global__ void __launch_bounds__(kTopkWarps * 32) li_topk_kernel(const SelectPa
 int launch_select(const SelectParams &sp, const BatchMeta &meta, cudaStream_t st, int64_t *n_launches) {
   {
     dim3 grid(sp.Nqb + sp.Mmax, sp.H, sp.B);
-    if (sp.d == 128) li_pool_kernel<128><<<grid, kPoolThreads, 0, st>>>(sp, meta);
-    else li_pool_kernel<64><<<grid, kPoolThreads, 0, st>>>(sp, meta);
+    if (sp.tl.bt > 0) {
+      if (sp.d == 128) li_pool_kernel<128, true><<<grid, kPoolThreads, 0, st>>>(sp, meta);
+      else li_pool_kernel<64, true><<<grid, kPoolThreads, 0, st>>>(sp, meta);
+    } else {
+      if (sp.d == 128) li_pool_kernel<128, false><<<grid, kPoolThreads, 0, st>>>(sp, meta);
+      else li_pool_kernel<64, false><<<grid, kPoolThreads, 0, st>>>(sp, meta);
+    }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return (int)e;
     if (n_launches) *n_launches += 1;

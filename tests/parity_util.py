@@ -21,7 +21,8 @@ def upload(prob: W.Problem, dev="cuda:0"):
     kc = prob.k_cache.to(dev)
     vc = prob.v_cache.to(dev)
     fi = torch.from_numpy(prob.frame_idx).to(dev)
-    ctx = li.Context(q, kc, vc, fi, prob.frame_off, prob.spec.n_cur_frames, prob.spec.block)
+    ctx = li.Context(q, kc, vc, fi, prob.frame_off, prob.spec.n_cur_frames, prob.spec.block,
+                     grid=prob.spec.grid, block3d=prob.spec.block3d)
     return ctx
 
 
@@ -70,12 +71,18 @@ def check_selection(prob: W.Problem, buf, oracle_sel, oracle_scores):
 
 def oracle_select(prob: W.Problem):
     s = prob.spec
+    if s.block3d is not None:
+        return O.block_select_3d(prob.u16(prob.q), prob.u16(prob.k_cache), prob.frame_idx, prob.frame_off,
+                                 s.n_cur_frames, *s.grid, *s.block3d, prob.top_k)
     return O.block_select(prob.u16(prob.q), prob.u16(prob.k_cache), prob.frame_idx, prob.frame_off,
                           s.n_cur_frames, s.block, s.block, prob.top_k)
 
 
 def oracle_attn(prob: W.Problem, sel_per_call, tiles=None):
     s = prob.spec
+    if s.block3d is not None:
+        return O.sparse_attn_3d(prob.u16(prob.q), prob.u16(prob.k_cache), prob.u16(prob.v_cache), prob.frame_idx,
+                                prob.frame_off, s.n_cur_frames, *s.grid, *s.block3d, sel_per_call, tiles=tiles)
     return O.sparse_attn(prob.u16(prob.q), prob.u16(prob.k_cache), prob.u16(prob.v_cache), prob.frame_idx,
                          prob.frame_off, s.n_cur_frames, s.block, s.block, sel_per_call, tiles=tiles)
 
@@ -94,6 +101,17 @@ def compare_output(o_gpu: torch.Tensor, lse_gpu, o_ref: np.ndarray, lse_ref: np.
             lg, lse_ref = lg[mask], lse_ref[mask]
         assert np.abs(lg - lse_ref).max() <= LSE_ABS, f"lse max-abs {np.abs(lg - lse_ref).max():.4g}"
     return float(diff.max()), float(diff.mean())
+
+
+def select_parity(prob: W.Problem):
+    """Mask + score parity of li_block_select alone."""
+    ctx = upload(prob)
+    buf = li.Buffers(ctx, prob.kmax, want_scores=True)
+    buf.sel_idx.fill_(-7)
+    li.li_block_select(ctx, prob.top_k, buf.kmax, buf.sel_idx, buf.sel_cnt, buf.workspace, buf.scores)
+    torch.cuda.synchronize()
+    osel, osc = oracle_select(prob)
+    return check_selection(prob, buf, osel, osc)
 
 
 def full_parity(prob: W.Problem):
