@@ -46,6 +46,22 @@ bool encode_map(CUtensorMap *tm, const void *base, int d, int64_t n1, int64_t n2
   return r == CUDA_SUCCESS;
 }
 
+// bf16 tensor viewed as 5-D [n4, n3, gh, gw, d] (innermost first: d, gw, gh, n3, n4), box = 64 x bw x bh x 1 x 1:
+// one frame's bh x bw patch of a 3-D block = 32 rows of 128 bytes, SWIZZLE_128B, zero fill outside.
+bool encode_map5(CUtensorMap *tm, const void *base, int d, int gw, int gh, int64_t n3, int64_t n4, int64_t s_w,
+                 int64_t s_h, int64_t s3, int64_t s4, int bw, int bh) {
+  EncodeFn enc = get_encode();
+  if (enc == nullptr) return false;
+  cuuint64_t dims[5] = {(cuuint64_t)d, (cuuint64_t)gw, (cuuint64_t)gh, (cuuint64_t)n3, (cuuint64_t)n4};
+  cuuint64_t strides[4] = {(cuuint64_t)s_w * 2, (cuuint64_t)s_h * 2, (cuuint64_t)s3 * 2, (cuuint64_t)s4 * 2};
+  cuuint32_t box[5] = {64, (cuuint32_t)bw, (cuuint32_t)bh, 1, 1};
+  cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+  CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 5, const_cast<void *>(base), dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS;
+}
+
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 inline size_t mpad(int m) { return m > 0 ? (size_t)((m + 31) & ~31) : 32; }   // row pitch of the transposed kbar
 
@@ -174,13 +190,27 @@ int li_sparse_attn(const li_problem *p, const int32_t *sel_idx, const int32_t *s
   const int half = blk / 2;                 // K/V are fetched as half-tiles of blk/2 rows
   const int has_full = p->frame_tokens >= half ? 1 : 0;
   CUtensorMap tm_q, tm_kf, tm_k8, tm_vf, tm_v8;
-  bool ok = encode_map(&tm_q, p->q, p->d, p->Lq, p->H, p->B, p->q_st, p->q_sh, p->q_sb, blk);
-  ok = ok && encode_map(&tm_k8, p->k_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp, 8);
-  ok = ok && encode_map(&tm_v8, p->v_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp, 8);
-  ok = ok && encode_map(&tm_kf, p->k_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp,
-                        has_full ? half : 8);
-  ok = ok && encode_map(&tm_vf, p->v_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp,
-                        has_full ? half : 8);
+  bool ok;
+  if (dv.tl.bt > 0) {
+    // 3-D blocks: 5-D maps (d, grid column, grid row, head | frame, page | batch*head)
+    const int gw = p->grid_w, gh = p->grid_h;
+    ok = encode_map5(&tm_q, p->q, p->d, gw, gh, p->Lq / p->frame_tokens, (int64_t)p->B * p->H, p->q_st, gw * p->q_st,
+                     (int64_t)p->frame_tokens * p->q_st, p->q_sh, p->bw, p->bh);
+    ok = ok && encode_map5(&tm_kf, p->k_cache, p->d, gw, gh, p->H, p->n_pages, p->kv_st, gw * p->kv_st, p->kv_sh,
+                           p->kv_sp, p->bw, p->bh);
+    ok = ok && encode_map5(&tm_vf, p->v_cache, p->d, gw, gh, p->H, p->n_pages, p->kv_st, gw * p->kv_st, p->kv_sh,
+                           p->kv_sp, p->bw, p->bh);
+    tm_k8 = tm_kf;
+    tm_v8 = tm_vf;
+  } else {
+    ok = encode_map(&tm_q, p->q, p->d, p->Lq, p->H, p->B, p->q_st, p->q_sh, p->q_sb, blk);
+    ok = ok && encode_map(&tm_k8, p->k_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp, 8);
+    ok = ok && encode_map(&tm_v8, p->v_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp, 8);
+    ok = ok && encode_map(&tm_kf, p->k_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp,
+                          has_full ? half : 8);
+    ok = ok && encode_map(&tm_vf, p->v_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp,
+                          has_full ? half : 8);
+  }
   if (!ok) return LI_ERR_CUDA;
 
   li::AttnParams ap;

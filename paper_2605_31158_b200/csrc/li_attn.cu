@@ -75,6 +75,7 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
   int32_t *sPages = reinterpret_cast<int32_t *>(smem + L::kOffPages);
   const uint32_t bar0 = smem_base + L::kOffBar;
   uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + L::kOffBar + 8 * BAR_COUNT);
+  int *sT = reinterpret_cast<int *>(smem + L::kOffBar + 8 * BAR_COUNT + 8);   // half-tile count (3-D mode)
   auto bar = [&](int i) { return bar0 + 8u * i; };
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -86,8 +87,13 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
   const int n_hist = n_frames - p.n_cur;
   const int L_hist = n_hist * p.T_f;
   const int L_cur = p.n_cur * p.T_f;
-  const int M = (L_hist + BLK - 1) / BLK;
-  const int Nc = (L_cur + BLK - 1) / BLK;
+  const Tiling tl = p.tl;
+  const bool k3d = tl.bt > 0;                          // 3-D blocks: BLK = bt*32, 32 = bh*bw rows per frame slice
+  constexpr int SPH = HALF / 32;                       // 32-row slices per half-tile
+  const int per = tl.Hb * tl.Wb;                       // blocks per temporal group (3-D)
+  const int M = tl.num_blocks(n_hist, p.T_f, BLK);
+  const int Nc = tl.num_blocks(p.n_cur, p.T_f, BLK);
+  const int n_qf = p.Lq / p.T_f;                       // query frames (3-D)
   const int64_t row_id = ((int64_t)b * p.H + h) * p.Nqb + i;
   const int valid_q = min(BLK, p.Lq - i * BLK);
   const int tail_cur = L_cur - (Nc - 1) * BLK, tail_hist = L_hist - (M - 1) * BLK;
@@ -100,6 +106,7 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
     tma_prefetch_desc(&tm_k_8);
     tma_prefetch_desc(&tm_v_8);
     for (int k = 0; k < BAR_COUNT; ++k) mbar_init(bar(k), (k == BAR_P_FULL || k == BAR_P_FULL + 1) ? 4 : 1);
+    *sT = 0;
     mbar_fence_init();
     fence_proxy_async();
   }
@@ -122,15 +129,41 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
 
   auto sel_at = [&](int jj) -> int { return jj < kSelCap ? sSel[jj] : sel_row[jj]; };
   auto page_at = [&](int f) -> int { return f < kPageCap ? sPages[f] : p.frame_idx[foff + f]; };
-  // valid key columns of attended tile j (chunk blocks first, then the selected historical blocks).  Only two tiles
-  // can be partial: the last chunk block, and the history tail block M-1, which (indices ascending) can only be the
-  // last selected one -- so no per-tile lookup is needed.
+  // ---- attended tile j (chunk blocks first, then the selected historical blocks) ----
+  // 1-D: only two tiles can be partial: the last chunk block, and the history tail block M-1, which (indices
+  // ascending) can only be the last selected one.  3-D: tiles of a region's last temporal group may hold fewer than
+  // bt frames, border tiles fewer than bh grid rows.
   const int j_tail_hist = (cnt > 0 && sel_at(cnt - 1) == M - 1) ? n_tiles - 1 : -1;
   auto tile_valid = [&](int j) -> int { return j == Nc - 1 ? tail_cur : (j == j_tail_hist ? tail_hist : BLK); };
+  auto tile_blk = [&](int j) -> int { return j < Nc ? j : sel_at(j - Nc); };
+  auto tile_frames = [&](int j) -> int {               // 3-D: frames of tile j that exist
+    return min(tl.bt, (j < Nc ? p.n_cur : n_hist) - (tile_blk(j) / per) * tl.bt);
+  };
+  auto halves = [&](int j) -> int {                    // half-tiles of tile j with at least one valid key
+    return k3d ? (tile_frames(j) > SPH ? 2 : 1) : (tile_valid(j) > HALF ? 2 : 1);
+  };
   // number of half-tiles with at least one valid key (a half-tile without any is skipped by every role)
   int T = 2 * n_tiles;
-  if (Nc > 0 && tail_cur <= HALF) --T;
-  if (j_tail_hist >= 0 && tail_hist <= HALF) --T;
+  if (k3d) {
+    int part = 0;
+    for (int j = threadIdx.x; j < n_tiles; j += blockDim.x) part += halves(j);
+    if (part) atomicAdd(sT, part);
+    __syncthreads();
+    T = *sT;
+  } else {
+    if (Nc > 0 && tail_cur <= HALF) --T;
+    if (j_tail_hist >= 0 && tail_hist <= HALF) --T;
+  }
+
+  // linear token of query row `row` of this tile, or -1 for a padding row ("masked stores")
+  auto row_token = [&](int row) -> int64_t {
+    if (k3d) {
+      const int tg = i / per, hb = (i - tg * per) / tl.Wb, wb = i - tg * per - hb * tl.Wb;
+      const int f = tg * tl.bt + (row >> 5), within = row & 31, y = hb * tl.bh + within / tl.bw;
+      return (row < BLK && f < n_qf && y < tl.gh) ? (int64_t)f * p.T_f + y * tl.gw + wb * tl.bw + within % tl.bw : -1;
+    }
+    return row < valid_q ? (int64_t)i * BLK + row : -1;
+  };
 
   if (T > 0) {
     if (warp == 4) {
@@ -139,7 +172,17 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
       if (elect_one()) {
         mbar_arrive_expect_tx(bar(BAR_Q_FULL), BLK * D * 2);
 #pragma unroll
-        for (int c = 0; c < D / 64; ++c) tma_load_4d(sQ + c * L::kQChunk, &tm_q, bar(BAR_Q_FULL), c * 64, i * BLK, h, b);
+        for (int c = 0; c < D / 64; ++c) {
+          if (k3d) {
+            // query block i = (tg, hb, wb): one 32-row box per frame; a frame past the chunk is out of bounds -> zeros
+            const int tg = i / per, hb = (i - tg * per) / tl.Wb, wb = i - tg * per - hb * tl.Wb;
+            for (int tt = 0; tt < BLK / 32; ++tt)
+              tma_load_5d(sQ + c * L::kQChunk + tt * 4096, &tm_q, bar(BAR_Q_FULL), c * 64, wb * tl.bw, hb * tl.bh,
+                          min(tg * tl.bt + tt, n_qf), b * p.H + h);
+          } else {
+            tma_load_4d(sQ + c * L::kQChunk, &tm_q, bar(BAR_Q_FULL), c * 64, i * BLK, h, b);
+          }
+        }
       }
       __syncwarp();
       int n = 0;                                     // running load index: slot = n % 4
@@ -148,10 +191,36 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
         const bool is_cur = j < Nc;
         const int blk = is_cur ? j : sel_at(j - Nc);
         const int f0 = is_cur ? n_hist : 0;            // first frame of the region inside this call's frame list
-        const int region_len = is_cur ? L_cur : L_hist;
-        const int t0 = blk * BLK + hh * HALF;
         const int slot = n & (kStages - 1);
         const uint32_t dst = sRing + slot * L::kStage, mb = bar(BAR_FULL + slot);
+        if (k3d) {
+          // 3-D block (tg, hb, wb): the half-tile is SPH frame slices of 32 rows (bh grid rows x bw columns), each one
+          // 5-D box (64 channels, bw, bh, head, page); grid rows >= grid_h are zero-filled by the hardware ("masked
+          // loads"); a frame past the region's end is requested out of bounds -> zeros
+          const int n_reg = is_cur ? p.n_cur : n_hist;
+          const int tg = blk / per, hb = (blk - tg * per) / tl.Wb, wb = blk - tg * per - hb * tl.Wb;
+          int pg[SPH], y0[SPH];
+#pragma unroll
+          for (int s = 0; s < SPH; ++s) {
+            const int f = tg * tl.bt + hh * SPH + s;
+            pg[s] = f < n_reg ? page_at(f0 + f) : 0;
+            y0[s] = f < n_reg ? hb * tl.bh : tl.gh;
+          }
+          mbar_wait(bar(BAR_EMPTY + slot), ((n >> 2) & 1) ^ 1);
+          if (elect_one()) {
+            mbar_arrive_expect_tx(mb, HALF * D * 2);
+#pragma unroll
+            for (int s = 0; s < SPH; ++s)
+#pragma unroll
+              for (int c = 0; c < D / 64; ++c)
+                tma_load_5d(dst + c * L::kKVChunk + s * 4096, tm_full, mb, c * 64, wb * tl.bw, y0[s], h, pg[s]);
+          }
+          __syncwarp();
+          ++n;
+          return;
+        }
+        const int region_len = is_cur ? L_cur : L_hist;
+        const int t0 = blk * BLK + hh * HALF;
         const int t_last = min(t0 + HALF, region_len) - 1;
         const int pg0 = t0 / p.T_f;
         const bool one_page = p.has_box_full && pg0 == t_last / p.T_f;
@@ -186,7 +255,7 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
         ++n;
       };
       auto advance = [&](int &j, int &hh) {
-        if (hh == 0 && tile_valid(j) > HALF) hh = 1;
+        if (hh == 0 && halves(j) > 1) hh = 1;
         else { ++j; hh = 0; }
       };
 
@@ -256,9 +325,24 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
       int j = 0, hh = 0;
 
       for (int t = 0; t < T; ++t) {
-        const int tv = tile_valid(j);
-        const int hv = min(HALF, tv - hh * HALF);      // valid key columns of this half-tile (> 0)
-        if (hh == 0 && tv > HALF) hh = 1;
+        // valid key columns of this half-tile, as a prefix length per 32-column slice (vs[s] rows of slice s are real,
+        // the rest is padding): 1-D blocks have one valid prefix; a 3-D slice is one frame's bh x bw patch, whose
+        // grid rows beyond grid_h (and whose frame, beyond the region) are padding
+        int vs[SPH];
+        if (k3d) {
+          const int blk = tile_blk(j), nf = tile_frames(j);
+          const int vrow = min(tl.bh, tl.gh - ((blk % per) / tl.Wb) * tl.bh) * tl.bw;
+#pragma unroll
+          for (int s_ = 0; s_ < SPH; ++s_) vs[s_] = (hh * SPH + s_ < nf) ? vrow : 0;
+        } else {
+          const int hv = min(HALF, tile_valid(j) - hh * HALF);
+#pragma unroll
+          for (int s_ = 0; s_ < SPH; ++s_) vs[s_] = min(32, max(0, hv - 32 * s_));
+        }
+        bool full = true;
+#pragma unroll
+        for (int s_ = 0; s_ < SPH; ++s_) full = full && vs[s_] == 32;
+        if (hh == 0 && halves(j) > 1) hh = 1;
         else { ++j; hh = 0; }
         const uint32_t s_addr = tmem + lane_base + (t & 1) * kSbCol;
 
@@ -268,9 +352,9 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
 #pragma unroll
         for (int c = 0; c < HALF / 32; ++c) tmem_ld32(s_addr + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&s[c * 32]));
         tc_wait_ld();
-        if (hv < HALF) {                               // padded key columns -> -inf (warp-uniform branch)
+        if (!full) {                                   // padded key columns -> -inf (warp-uniform branch)
 #pragma unroll
-          for (int c = 0; c < HALF; ++c) if (c >= hv) s[c] = 0xff800000u;
+          for (int c = 0; c < HALF; ++c) if ((c & 31) >= vs[c >> 5]) s[c] = 0xff800000u;
         }
         float mx0 = __uint_as_float(s[0]), mx1 = __uint_as_float(s[1]), mx2 = __uint_as_float(s[2]), mx3 = __uint_as_float(s[3]);
 #pragma unroll
@@ -341,8 +425,9 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
       mbar_wait(bar(BAR_O_FULL), 0);
       tc_fence_after();
       const float inv_l = 1.0f / l;
-      const bool live = row < valid_q;
-      uint16_t *orow = p.o + (((int64_t)b * p.H + h) * p.Lq + (int64_t)i * BLK + row) * D;
+      const int64_t u = row_token(row);
+      const bool live = u >= 0;
+      uint16_t *orow = p.o + (((int64_t)b * p.H + h) * p.Lq + u) * D;
 #pragma unroll
       for (int c = 0; c < D / 32; ++c) {
         uint32_t o[32];
@@ -361,16 +446,16 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
         }
       }
       if (live && p.lse != nullptr)
-        p.lse[((int64_t)b * p.H + h) * p.Lq + (int64_t)i * BLK + row] = (m_used + log2f(l)) * 0.6931471805599453f;
+        p.lse[((int64_t)b * p.H + h) * p.Lq + u] = (m_used + log2f(l)) * 0.6931471805599453f;
     }
   } else {
     // empty context: o = 0, lse = -inf
     if (warp < 4) {
-      const int row = warp * 32 + lane;
-      if (row < valid_q) {
-        uint16_t *orow = p.o + (((int64_t)b * p.H + h) * p.Lq + (int64_t)i * BLK + row) * D;
+      const int64_t u = row_token(warp * 32 + lane);
+      if (u >= 0) {
+        uint16_t *orow = p.o + (((int64_t)b * p.H + h) * p.Lq + u) * D;
         for (int c = 0; c < D; c += 8) *reinterpret_cast<uint4 *>(orow + c) = make_uint4(0, 0, 0, 0);
-        if (p.lse != nullptr) p.lse[((int64_t)b * p.H + h) * p.Lq + (int64_t)i * BLK + row] = __int_as_float(0xff800000);
+        if (p.lse != nullptr) p.lse[((int64_t)b * p.H + h) * p.Lq + u] = __int_as_float(0xff800000);
       }
     }
   }
