@@ -105,20 +105,20 @@ def oracle_sample(prob: W.Problem, n_heads: int, tiles_per_head=None):
     if tiles_per_head is not None:
         tiles = [(0, h, i) for h in range(nh) for i in range(nq)]
     t0 = time.perf_counter()
-    sel, _ = O.block_select(q, kc, fi, fo, s.n_cur_frames, s.block, s.block, prob.top_k[:1])
-    O.sparse_attn(q, kc, vc, fi, fo, s.n_cur_frames, s.block, s.block, sel, tiles=tiles)
+    if s.block3d is not None:
+        sel, _ = O.block_select_3d(q, kc, fi, fo, s.n_cur_frames, *s.grid, *s.block3d, prob.top_k[:1])
+        O.sparse_attn_3d(q, kc, vc, fi, fo, s.n_cur_frames, *s.grid, *s.block3d, sel, tiles=tiles)
+    else:
+        sel, _ = O.block_select(q, kc, fi, fo, s.n_cur_frames, s.block, s.block, prob.top_k[:1])
+        O.sparse_attn(q, kc, vc, fi, fo, s.n_cur_frames, s.block, s.block, sel, tiles=tiles)
     dt = time.perf_counter() - t0
     sub = W.Problem(s, prob.q[:1, :nh], prob.k_cache, prob.v_cache, fi, fo, prob.top_k[:1])
-    cnt = np.full((nh, prob.Nqb), sel[0].shape[-1], np.int32)
-    flops = 0
+    vq, vk = sub.block_sizes(s.n_cur_frames), sub.block_sizes(sub.n_hist_frames(0))   # valid tokens per block
     Lc = s.n_cur_frames * s.frame_tokens
-    Lh, M = sub.L_hist(0), sub.M(0)
-    tail = Lh - (M - 1) * s.block if M > 0 else 0
+    flops = 0
     for h in range(nh):
         for i in range(nq):
-            vq = min(s.block, sub.Lq - i * s.block)
-            kv = Lc + sum((tail if int(m) == M - 1 else s.block) for m in sel[0][h, i])
-            flops += 4 * s.d * vq * kv
+            flops += 4 * s.d * int(vq[i]) * (Lc + int(sum(vk[int(m)] for m in sel[0][h, i])))
     desc = f"{s.name}: call 0, heads 0..{nh - 1} of {s.H}, query blocks 0..{nq - 1} of {prob.Nqb}, select + attention"
     return dt, flops, desc
 
@@ -206,7 +206,7 @@ def run_cuda(args):
     kc = prob.k_cache.to(dev)
     vc = prob.v_cache.to(dev)
     fi = torch.from_numpy(prob.frame_idx).to(dev)
-    ctx = li.Context(q, kc, vc, fi, prob.frame_off, s.n_cur_frames, s.block)
+    ctx = li.Context(q, kc, vc, fi, prob.frame_off, s.n_cur_frames, s.block, grid=s.grid, block3d=s.block3d)
     buf = li.Buffers(ctx, prob.kmax, want_scores=False, want_lse=True)
     o_host = torch.empty(buf.o.shape, dtype=buf.o.dtype).pin_memory()
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)   # > 126 MB L2
@@ -306,7 +306,7 @@ def run_cuda(args):
         if need_b < free_b // 2:
             kc2, vc2 = kc.index_select(0, order), vc.index_select(0, order)
             ident = torch.arange(order.numel(), dtype=torch.int32, device=dev)
-            ctx2 = li.Context(q, kc2, vc2, ident, prob.frame_off, s.n_cur_frames, s.block)
+            ctx2 = li.Context(q, kc2, vc2, ident, prob.frame_off, s.n_cur_frames, s.block, grid=s.grid, block3d=s.block3d)
             t_paged, t_ident = time_attn(ctx), time_attn(ctx2)
             extras["attn_ms_paged"] = t_paged
             extras["attn_ms_identity_contiguous"] = t_ident
@@ -325,7 +325,7 @@ def run_cuda(args):
             "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "bf16", "data": "synthetic",
             "config": {"workload": s.name, "B": prob.B, "H": s.H, "d": s.d, "Lq": prob.Lq, "frame_tokens": s.frame_tokens,
-                       "block": s.block, "Lk": [prob.L_hist(b) + prob.Lq for b in range(prob.B)],
+                       "block": s.block, "block3d": s.block3d, "grid": s.grid, "Lk": [prob.L_hist(b) + prob.Lq for b in range(prob.B)],
                        "top_k": [int(x) for x in prob.top_k], "M": [prob.M(b) for b in range(prob.B)],
                        "l2": "flushed between timed steps (256 MiB write)", "multi_gpu": "replicas only (no collective)"},
             "effective_flops_per_step": int(flops),
@@ -362,7 +362,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--config", default="mid", choices=["tiny", "mid", "long", "adaptive", "dense-equivalence"])
+    ap.add_argument("--config", default="mid", choices=["tiny", "mid", "long", "adaptive", "dense-equivalence", "mid3d"])
     ap.add_argument("--ref-heads", type=int, default=24, help="heads in the oracle's bounded sample")
     ap.add_argument("--ref-tiles", type=int, default=None, help="query blocks per head in the oracle's sample (default all)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")

@@ -22,6 +22,7 @@
 
 namespace li {
 
+constexpr int kInfoCap = 2048;      // attended tiles whose 3-D geometry is tabulated in shared memory
 constexpr int kPageCap = 256;       // frame-list entries staged in shared memory (rest read from global)
 constexpr int kSelCap = 1024;       // selected-block indices staged in shared memory (rest read from global)
 constexpr int kTmemCols = 256;
@@ -45,7 +46,8 @@ struct AttnSmem {
   static constexpr int kOffRing = kQ;
   static constexpr int kOffSel = kQ + kStages * kStage;
   static constexpr int kOffPages = kOffSel + kSelCap * 4;   // this call's frame list, staged once
-  static constexpr int kOffBar = kOffPages + kPageCap * 4;
+  static constexpr int kOffInfo = kOffPages + kPageCap * 4;  // 3-D: per attended tile (frames present) | (valid rows per slice) << 8
+  static constexpr int kOffBar = kOffInfo + kInfoCap * 2;
   static constexpr int kTotal = kOffBar + 256 + 1024;  // + barriers + slack for 1024-B alignment
 };
 
@@ -60,7 +62,7 @@ enum {
   BAR_COUNT
 };
 
-template <int D, int BLK>
+template <int D, int BLK, bool K3D>
 __global__ void __launch_bounds__(192, 2)
 li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_constant__ CUtensorMap tm_q,
                       const __grid_constant__ CUtensorMap tm_k_full, const __grid_constant__ CUtensorMap tm_k_8,
@@ -73,6 +75,7 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
   const uint32_t sQ = smem_base + L::kOffQ, sRing = smem_base + L::kOffRing;
   int32_t *sSel = reinterpret_cast<int32_t *>(smem + L::kOffSel);
   int32_t *sPages = reinterpret_cast<int32_t *>(smem + L::kOffPages);
+  uint16_t *sInfo = reinterpret_cast<uint16_t *>(smem + L::kOffInfo);
   const uint32_t bar0 = smem_base + L::kOffBar;
   uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + L::kOffBar + 8 * BAR_COUNT);
   int *sT = reinterpret_cast<int *>(smem + L::kOffBar + 8 * BAR_COUNT + 8);   // half-tile count (3-D mode)
@@ -88,7 +91,7 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
   const int L_hist = n_hist * p.T_f;
   const int L_cur = p.n_cur * p.T_f;
   const Tiling tl = p.tl;
-  const bool k3d = tl.bt > 0;                          // 3-D blocks: BLK = bt*32, 32 = bh*bw rows per frame slice
+  constexpr bool k3d = K3D;                            // 3-D blocks: BLK = bt*32, 32 = bh*bw rows per frame slice
   constexpr int SPH = HALF / 32;                       // 32-row slices per half-tile
   const int per = tl.Hb * tl.Wb;                       // blocks per temporal group (3-D)
   const int M = tl.num_blocks(n_hist, p.T_f, BLK);
@@ -136,9 +139,13 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
   const int j_tail_hist = (cnt > 0 && sel_at(cnt - 1) == M - 1) ? n_tiles - 1 : -1;
   auto tile_valid = [&](int j) -> int { return j == Nc - 1 ? tail_cur : (j == j_tail_hist ? tail_hist : BLK); };
   auto tile_blk = [&](int j) -> int { return j < Nc ? j : sel_at(j - Nc); };
-  auto tile_frames = [&](int j) -> int {               // 3-D: frames of tile j that exist
-    return min(tl.bt, (j < Nc ? p.n_cur : n_hist) - (tile_blk(j) / per) * tl.bt);
+  auto tile_info = [&](int j) -> int {                 // 3-D: (frames of tile j that exist) | (valid rows per slice) << 8
+    const int blk = tile_blk(j);
+    const int nf = min(tl.bt, (j < Nc ? p.n_cur : n_hist) - (blk / per) * tl.bt);
+    return nf | (min(tl.bh, tl.gh - ((blk % per) / tl.Wb) * tl.bh) * tl.bw) << 8;
   };
+  auto tile_info_cached = [&](int j) -> int { return j < kInfoCap ? (int)sInfo[j] : tile_info(j); };
+  auto tile_frames = [&](int j) -> int { return tile_info_cached(j) & 0xff; };
   auto halves = [&](int j) -> int {                    // half-tiles of tile j with at least one valid key
     return k3d ? (tile_frames(j) > SPH ? 2 : 1) : (tile_valid(j) > HALF ? 2 : 1);
   };
@@ -146,7 +153,11 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
   int T = 2 * n_tiles;
   if (k3d) {
     int part = 0;
-    for (int j = threadIdx.x; j < n_tiles; j += blockDim.x) part += halves(j);
+    for (int j = threadIdx.x; j < n_tiles; j += blockDim.x) {
+      const int info = tile_info(j);                   // integer divisions once per tile, not once per half-tile per role
+      if (j < kInfoCap) sInfo[j] = (uint16_t)info;
+      part += (info & 0xff) > SPH ? 2 : 1;
+    }
     if (part) atomicAdd(sT, part);
     __syncthreads();
     T = *sT;
@@ -330,8 +341,7 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
         // grid rows beyond grid_h (and whose frame, beyond the region) are padding
         int vs[SPH];
         if (k3d) {
-          const int blk = tile_blk(j), nf = tile_frames(j);
-          const int vrow = min(tl.bh, tl.gh - ((blk % per) / tl.Wb) * tl.bh) * tl.bw;
+          const int info = tile_info_cached(j), nf = info & 0xff, vrow = info >> 8;
 #pragma unroll
           for (int s_ = 0; s_ < SPH; ++s_) vs[s_] = (hh * SPH + s_ < nf) ? vrow : 0;
         } else {
@@ -465,11 +475,11 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
   if (warp == 5) tmem_dealloc(tmem, kTmemCols);
 }
 
-template <int D, int BLK>
+template <int D, int BLK, bool K3D>
 static int launch_one(const AttnParams &ap, const BatchMeta &meta, const CUtensorMap &tm_q, const CUtensorMap &tm_k_full,
                       const CUtensorMap &tm_k_8, const CUtensorMap &tm_v_full, const CUtensorMap &tm_v_8,
                       cudaStream_t st) {
-  auto kern = li_sparse_attn_kernel<D, BLK>;
+  auto kern = li_sparse_attn_kernel<D, BLK, K3D>;
   constexpr int smem = AttnSmem<D, BLK>::kTotal;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   if (e != cudaSuccess) return (int)e;
@@ -492,10 +502,15 @@ int launch_attn(const AttnParams &ap, const BatchMeta &meta, int d, int blk, con
                 const CUtensorMap &tm_k_full, const CUtensorMap &tm_k_8, const CUtensorMap &tm_v_full,
                 const CUtensorMap &tm_v_8, cudaStream_t st, int64_t *n_launches) {
   int e;
-  if (d == 128 && blk == 128) e = launch_one<128, 128>(ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st);
-  else if (d == 128 && blk == 64) e = launch_one<128, 64>(ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st);
-  else if (d == 64 && blk == 128) e = launch_one<64, 128>(ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st);
-  else e = launch_one<64, 64>(ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st);
+  const bool k3 = ap.tl.bt > 0;
+#define LI_LAUNCH(DD, BB)                                                                                  \
+  (k3 ? launch_one<DD, BB, true>(ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st)                \
+      : launch_one<DD, BB, false>(ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st))
+  if (d == 128 && blk == 128) e = LI_LAUNCH(128, 128);
+  else if (d == 128 && blk == 64) e = LI_LAUNCH(128, 64);
+  else if (d == 64 && blk == 128) e = LI_LAUNCH(64, 128);
+  else e = LI_LAUNCH(64, 64);
+#undef LI_LAUNCH
   if (e == 0 && n_launches) *n_launches += 1;
   return e;
 }

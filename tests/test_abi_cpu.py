@@ -100,6 +100,33 @@ def test_workspace_bytes_and_validation(L):
     assert L.li_block_select(None, tk.ctypes.data, 8, 1, 1, None, 0, 1, 1, None) == li.LI_ERR_INVALID_ARG
 
 
+def test_3d_tiling_validation(L):
+    """3-D block fields: accepted geometries and host-side rejections."""
+    def prob3d(**over):
+        fo = np.asarray([0, 6], dtype=np.int32)
+        p, _ = make_problem(frame_tokens=30 * 52, Lq=2 * 30 * 52, d=128, block_q=128, block_k=128, n_cur_frames=2,
+                            q_sb=24 * 3120 * 128, q_sh=3120 * 128, q_st=128, kv_sp=24 * 1560 * 128, kv_sh=1560 * 128,
+                            kv_st=128, H=24, grid_h=30, grid_w=52, bt=4, bh=8, bw=4)
+        p.frame_off_host = fo.ctypes.data
+        for k, v in over.items():
+            setattr(p, k, v)
+        return p, fo
+    p, keep = prob3d()
+    # history 4 frames -> 1 temporal group x 4 x 13 = 52 blocks; Nqb = 52 (chunk of 2 frames = one partial group)
+    ws = L.li_workspace_bytes(ctypes.byref(p), 8)
+    assert ws == 24 * 52 * 128 * 4 + 24 * 128 * 64 * 4 + 24 * 52 * 52 * 4 + (256 - (24 * 52 * 52 * 4) % 256) % 256
+    for bad, code in ((dict(bw=8), li.LI_ERR_UNSUPPORTED),            # 4*8*8 != 128
+                      (dict(bh=4, bw=8), li.LI_ERR_UNSUPPORTED),       # 52 % 8 != 0
+                      (dict(grid_w=50), li.LI_ERR_INVALID_ARG),        # grid_h*grid_w != frame_tokens
+                      (dict(bt=0), li.LI_ERR_INVALID_ARG),             # partially specified
+                      (dict(bt=2, block_q=64, block_k=64), li.LI_OK)): # (2,8,4) = 64-token blocks
+        pb, keep2 = prob3d(**bad)
+        got = L.li_workspace_bytes(ctypes.byref(pb), 8)
+        assert (got > 0) == (code == li.LI_OK), bad
+        if code != li.LI_OK:
+            assert L.li_sparse_attn(ctypes.byref(pb), 0x60000, 0x70000, 8, 0x80000, None, None, 0, None) == code, bad
+
+
 def test_binding_refuses_cpu_tensors():
     import torch
     q = torch.zeros((1, 2, 256, 64), dtype=torch.bfloat16)
