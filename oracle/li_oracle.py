@@ -28,8 +28,9 @@ means of constant blocks, ragged tails, NaN padding; closed-form ranking; argsor
 force; exact ties -> lowest index; k=M; nested selections.
 The 3-D block tiling of PAPER.md:129/:321 (functions *_3d at the end) is pinned by tests/test_oracle_3d_pins.py:
 explicit coordinate brute force, reduction to the 1-D tiling when blocks are row segments, partition and padding
-properties.  Nothing in this file is "parity unpinned".  (Text prefix and the policy scalars of Eq. 1-8 are not
-implemented here at all: out of the hot-path scope.)
+properties.  The text set T of Eq. 11 (text_k / text_v arguments) is pinned in the same files (brute force, dense SDPA over
+[text | context], text-only attention).  Nothing in this file is "parity unpinned".  (The policy scalars of Eq. 1-8
+are not implemented here at all: out of the hot-path scope.)
 """
 from __future__ import annotations
 
@@ -149,11 +150,13 @@ def softmax_attend(qr: np.ndarray, K: np.ndarray, V: np.ndarray, scale: float):
 
 def sparse_attn(q, k_cache, v_cache, frame_idx, frame_off, n_cur_frames: int, block_q: int,
                 block_k: int, sel_idx: Sequence[np.ndarray], softmax_scale: float = 0.0,
-                tiles: Optional[Sequence[Tuple[int, int, int]]] = None):
+                tiles: Optional[Sequence[Tuple[int, int, int]]] = None, text_k=None, text_v=None):
     """li_sparse_attn: step 6 for every (call, head, query block), or only for `tiles`
     = [(b, h, i), ...] (sampled parity at full size).  sel_idx[b]: int [H,Nqb,k_b]; negative
     entries are padding.  Query block i attends ALL chunk tokens (K^curr, no mask inside the
-    chunk: DESIGN.md c8) plus the valid tokens of its selected history blocks.
+    chunk: DESIGN.md c8) plus the valid tokens of its selected history blocks, plus -- when text_k / text_v
+    [B,H,Lt,d] are given -- ALL text-conditioning tokens: C_i = T U K^curr U S_i (Eq. 11, PAPER.md:142-144;
+    "the model retains all text-conditioning tokens", PAPER.md:129).
     Returns o fp32 [B,H,Lq,d], lse fp32 [B,H,Lq]  (untouched tiles stay NaN when `tiles`)."""
     B, H, Lq, d = q.shape
     scale = softmax_scale if softmax_scale != 0.0 else 1.0 / math.sqrt(d)
@@ -174,6 +177,9 @@ def sparse_attn(q, k_cache, v_cache, frame_idx, frame_off, n_cur_frames: int, bl
         t = attended_rows(Kh.shape[0], block_k, rows)
         K = np.concatenate([Kc, Kh[t]], axis=0)             # C_i = K^curr U S_i  (Eq. 11)
         V = np.concatenate([Vc, Vh[t]], axis=0)             # same indices for K and V
+        if text_k is not None:                              # ... U T: the text tokens are always kept (Eq. 11)
+            K = np.concatenate([widen(text_k[b, h]), K], axis=0)
+            V = np.concatenate([widen(text_v[b, h]), V], axis=0)
         u0, u1 = i * block_q, min(Lq, (i + 1) * block_q)
         oi, li = softmax_attend(widen(q[b, h, u0:u1]), K, V, scale)
         o[b, h, u0:u1] = oi.astype(np.float32)
@@ -251,7 +257,7 @@ def block_select_3d(q, k_cache, frame_idx, frame_off, n_cur_frames: int, grid_h:
 
 def sparse_attn_3d(q, k_cache, v_cache, frame_idx, frame_off, n_cur_frames: int, grid_h: int, grid_w: int, bt: int,
                    bh: int, bw: int, sel_idx: Sequence[np.ndarray], softmax_scale: float = 0.0,
-                   tiles: Optional[Sequence[Tuple[int, int, int]]] = None):
+                   tiles: Optional[Sequence[Tuple[int, int, int]]] = None, text_k=None, text_v=None):
     """li_sparse_attn with 3-D blocks: the queries of 3-D query block i attend ALL chunk tokens plus the valid tokens
     of the selected 3-D history blocks; outputs in the original linear token order."""
     B, H, Lq, d = q.shape
@@ -274,6 +280,9 @@ def sparse_attn_3d(q, k_cache, v_cache, frame_idx, frame_off, n_cur_frames: int,
         t = np.concatenate([kblocks[m] for m in rows]) if rows else np.zeros((0,), dtype=np.int64)
         K = np.concatenate([Kc, Kh[t]], axis=0)
         V = np.concatenate([Vc, Vh[t]], axis=0)
+        if text_k is not None:                              # T of Eq. 11: always kept
+            K = np.concatenate([widen(text_k[b, h]), K], axis=0)
+            V = np.concatenate([widen(text_v[b, h]), V], axis=0)
         u = qblocks[i]
         oi, li = softmax_attend(widen(q[b, h])[u], K, V, scale)
         o[b, h, u] = oi.astype(np.float32)

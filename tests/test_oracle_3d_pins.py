@@ -128,3 +128,50 @@ def test_all_blocks_is_dense_and_constant_v():
     sel2, _ = O.block_select_3d(q, kc, fi, fo, 2, 3, 4, 2, 2, 3, [4])
     o2, _ = O.sparse_attn_3d(q, kc, np.broadcast_to(c, vc.shape).copy(), fi, fo, 2, 3, 4, 2, 2, 3, sel2)
     np.testing.assert_allclose(o2, np.broadcast_to(c, o2.shape), rtol=1e-6, atol=1e-6)
+
+
+# ----------------------------------------------------------------------------- text prefix T of Eq. 11
+def test_text_tokens_are_always_attended():
+    """C_i = T U K^curr U S_i: (i) with every block selected the result is dense SDPA over [text | whole context];
+    (ii) with no chunk and nothing selected it is SDPA over the text alone; (iii) a brute-force masked softmax in plain
+    loops for a partial selection; (iv) K and V of the text are not swapped (V indicator test)."""
+    q, kc, vc, fi, fo = rand_problem()
+    d = q.shape[-1]
+    Lt = 5
+    tk = RNG.standard_normal((1, 2, Lt, d)); tv = RNG.standard_normal((1, 2, Lt, d))
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a))[None]
+    sdpa = lambda qq, K, V: torch.nn.functional.scaled_dot_product_attention(t(qq), t(K), t(V))[0].numpy()
+    # (i) 1-D blocks, everything selected
+    Bk = 5
+    M = -(-5 * 12 // Bk)
+    sel, _ = O.block_select(q, kc, fi, fo, 2, Bk, Bk, [M])
+    o, _ = O.sparse_attn(q, kc, vc, fi, fo, 2, Bk, Bk, sel, text_k=tk, text_v=tv)
+    for h in range(2):
+        K = np.concatenate([tk[0, h]] + [kc[p, h] for p in fi]); V = np.concatenate([tv[0, h]] + [vc[p, h] for p in fi])
+        np.testing.assert_allclose(o[0, h], sdpa(q[0, h], K, V), rtol=1e-5, atol=1e-6)
+    # (ii) no chunk (n_cur = 0), nothing selected: text only
+    o2, _ = O.sparse_attn(q, kc, vc, fi, fo, 0, Bk, Bk, [np.zeros((2, 5, 0), np.int32)], text_k=tk, text_v=tv)
+    for h in range(2):
+        np.testing.assert_allclose(o2[0, h], sdpa(q[0, h], tk[0, h], tv[0, h]), rtol=1e-5, atol=1e-6)
+    # (iii) 3-D blocks, partial selection, brute force in loops
+    gh, gw, bt, bh, bw = 3, 4, 2, 2, 3
+    sel3, _ = O.block_select_3d(q, kc, fi, fo, 2, gh, gw, bt, bh, bw, [4])
+    o3, l3 = O.sparse_attn_3d(q, kc, vc, fi, fo, 2, gh, gw, bt, bh, bw, sel3, text_k=tk, text_v=tv)
+    bo, bl = brute_3d(q[0], kc, vc, list(fi), 2, gh, gw, bt, bh, bw, sel3[0], 1 / math.sqrt(d))
+    scale = 1 / math.sqrt(d)
+    for h in range(2):
+        for u in range(q.shape[2]):
+            st = scale * (tk[0, h] @ q[0, h, u])
+            lse_all = np.logaddexp(bl[h, u], np.log(np.exp(st - st.max()).sum()) + st.max())
+            w_ctx = math.exp(bl[h, u] - lse_all)
+            want = w_ctx * bo[h, u] + (np.exp(st - lse_all)[:, None] * tv[0, h]).sum(0)
+            np.testing.assert_allclose(o3[0, h, u], want, rtol=1e-5, atol=1e-6)
+            assert abs(l3[0, h, u] - lse_all) < 1e-5
+    # (iv) text K / V roles: only text token 3 matches the query, V is an indicator of the token id
+    q1 = np.zeros((1, 1, 12, 4)); q1[..., 0] = 60.0
+    tk1 = np.zeros((1, 1, 6, 4)); tk1[0, 0, 3, 0] = 1.0
+    tv1 = np.zeros((1, 1, 6, 4)); tv1[0, 0, 3, 2] = 1.0
+    z = np.zeros((2, 1, 12, 4))
+    o4, _ = O.sparse_attn(q1, z, z, np.asarray([0, 1], np.int32), np.asarray([0, 2], np.int32), 1, 4, 4,
+                          [np.zeros((1, 3, 0), np.int32)], text_k=tk1, text_v=tv1)
+    assert (o4[0, 0, :, 2] > 0.999).all()
