@@ -4,7 +4,7 @@
  * Two operations (PAPER.md = /root/reference/PAPER.md, cited by line):
  *   li_block_select : Eq. 9 block mean pooling of Q and of the historical K, per head;
  *                     Eq. 10 score qbar_i . kbar_m / sqrt(d) and Top_{floor(rM)} per query block.
- *   li_sparse_attn  : Eq. 11 context C_i = K^curr U S_i (text set T absent), then softmax
+ *   li_sparse_attn  : Eq. 11 context C_i = T U K^curr U S_i (T = optional text tokens), then softmax
  *                     attention of query block i over C_i ("sparse attention core").
  * The KV context is never materialised: K/V rows are read in place from a frame-paged cache through a
  * frame-index list  memory | temporal window | current chunk  (Fig. 2a "reconstruct the KV
@@ -71,6 +71,13 @@ typedef struct li_problem {
    * (q_sb == H*q_sh). */
   int32_t grid_h, grid_w;
   int32_t bt, bh, bw;
+  /* Text-conditioning tokens T of Eq. 11 (C_i = T U K^curr U S_i; "the model retains all
+   * text-conditioning tokens"): a dense, non-paged K/V region attended by every query, never pooled nor
+   * selected.  Lt == 0 (and NULL pointers) = no text. */
+  int32_t Lt;                   /* text tokens per call */
+  const void *text_k;           /* bf16 [B,H,Lt,d] */
+  const void *text_v;           /* bf16, same shape and strides */
+  int64_t t_sb, t_sh, t_st;     /* batch / head / token strides of both */
 } li_problem;
 
 /* Eq. 9-10.  For every call b, head h and query block i: pooled means (true cardinality
@@ -87,8 +94,8 @@ int li_block_select(const li_problem *p, const int32_t *top_k_host, int32_t kmax
                     int32_t *sel_idx, int32_t *sel_cnt, float *scores_opt, int32_t score_pitch,
                     void *workspace, size_t workspace_bytes, void *cuda_stream);
 
-/* Eq. 11 + attention.  Query block i of (b,h) attends ALL chunk tokens (bidirectional
- * inside the chunk) plus the valid tokens of historical blocks sel_idx[b,h,i,0..sel_cnt[b,h,i]); the same
+/* Eq. 11 + attention.  Query block i of (b,h) attends ALL text tokens (if any), ALL chunk tokens
+ * (bidirectional inside the chunk) plus the valid tokens of historical blocks sel_idx[b,h,i,0..sel_cnt[b,h,i]); the same
  * indices address K and V.  softmax in fp32 (online), bf16 tcgen05 MMAs with fp32 accumulation.
  *   o       : bf16 [B,H,Lq,d], contiguous.
  *   lse_opt : NULL or fp32 [B,H,Lq]: log sum_n exp(scale * q.k_n) (natural log).

@@ -42,6 +42,8 @@ class li_problem(ctypes.Structure):
         ("n_cur_frames", ctypes.c_int32), ("softmax_scale", ctypes.c_float),
         ("grid_h", ctypes.c_int32), ("grid_w", ctypes.c_int32),
         ("bt", ctypes.c_int32), ("bh", ctypes.c_int32), ("bw", ctypes.c_int32),
+        ("Lt", ctypes.c_int32), ("text_k", ctypes.c_void_p), ("text_v", ctypes.c_void_p),
+        ("t_sb", ctypes.c_int64), ("t_sh", ctypes.c_int64), ("t_st", ctypes.c_int64),
     ]
 
 
@@ -96,7 +98,8 @@ class Context:
 
     def __init__(self, q: torch.Tensor, k_cache: torch.Tensor, v_cache: torch.Tensor, frame_idx: torch.Tensor,
                  frame_off: Sequence[int], n_cur_frames: int, block: int, softmax_scale: float = 0.0,
-                 grid: Optional[Tuple[int, int]] = None, block3d: Optional[Tuple[int, int, int]] = None):
+                 grid: Optional[Tuple[int, int]] = None, block3d: Optional[Tuple[int, int, int]] = None,
+                 text_k: Optional[torch.Tensor] = None, text_v: Optional[torch.Tensor] = None):
         for t, name in ((q, "q"), (k_cache, "k_cache"), (v_cache, "v_cache")):
             if t.dtype != torch.bfloat16 or not t.is_cuda or t.dim() != 4 or t.stride(-1) != 1:
                 raise ValueError(f"{name} must be a 4-D CUDA bf16 tensor with unit innermost stride")
@@ -122,6 +125,16 @@ class Context:
         p.frame_off_host = self.frame_off.ctypes.data
         p.n_cur_frames = n_cur_frames
         p.softmax_scale = softmax_scale
+        self.text_k, self.text_v = text_k, text_v
+        if text_k is not None:
+            for t, name in ((text_k, "text_k"), (text_v, "text_v")):
+                if t.dtype != torch.bfloat16 or not t.is_cuda or t.dim() != 4 or t.stride(-1) != 1:
+                    raise ValueError(f"{name} must be a 4-D CUDA bf16 tensor with unit innermost stride")
+            if text_k.shape != text_v.shape or text_k.stride() != text_v.stride() or text_k.shape[:2] != (B, H):
+                raise ValueError("text_k / text_v must both be [B,H,Lt,d] with equal strides")
+            p.Lt = text_k.shape[2]
+            p.text_k, p.text_v = text_k.data_ptr(), text_v.data_ptr()
+            p.t_sb, p.t_sh, p.t_st = text_k.stride(0), text_k.stride(1), text_k.stride(2)
         self.p = p
         self.B, self.H, self.Lq, self.d, self.block = B, H, Lq, d, block
         n_hist = (self.frame_off[1:] - self.frame_off[:-1]) - n_cur_frames

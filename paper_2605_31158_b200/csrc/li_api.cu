@@ -90,6 +90,15 @@ int check_problem(const li_problem *p, Derived *dv) {
     if (s <= 0 || s % 8 != 0) return LI_ERR_INVALID_ARG;
   if (p->q_st < p->d || p->kv_st < p->d) return LI_ERR_INVALID_ARG;
   if (((uintptr_t)p->q | (uintptr_t)p->k_cache | (uintptr_t)p->v_cache) & 15u) return LI_ERR_INVALID_ARG;
+  if (p->Lt < 0) return LI_ERR_INVALID_ARG;
+  if (p->Lt > 0) {
+    if (p->text_k == nullptr || p->text_v == nullptr) return LI_ERR_INVALID_ARG;
+    if ((((uintptr_t)p->text_k | (uintptr_t)p->text_v) & 15u) != 0) return LI_ERR_INVALID_ARG;
+    const int64_t ts[3] = {p->t_sb, p->t_sh, p->t_st};
+    for (int64_t s : ts)
+      if (s <= 0 || s % 8 != 0) return LI_ERR_INVALID_ARG;
+    if (p->t_st < p->d) return LI_ERR_INVALID_ARG;
+  }
   std::memset(&dv->meta, 0, sizeof(dv->meta));
   std::memset(&dv->tl, 0, sizeof(dv->tl));
   const bool any3d = p->grid_h | p->grid_w | p->bt | p->bh | p->bw;
@@ -211,19 +220,24 @@ int li_sparse_attn(const li_problem *p, const int32_t *sel_idx, const int32_t *s
     ok = ok && encode_map(&tm_vf, p->v_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp,
                           has_full ? half : 8);
   }
+  CUtensorMap tm_tk = tm_q, tm_tv = tm_q;      // placeholders when there is no text
+  if (p->Lt > 0) {
+    ok = ok && encode_map(&tm_tk, p->text_k, p->d, p->Lt, p->H, p->B, p->t_st, p->t_sh, p->t_sb, half);
+    ok = ok && encode_map(&tm_tv, p->text_v, p->d, p->Lt, p->H, p->B, p->t_st, p->t_sh, p->t_sb, half);
+  }
   if (!ok) return LI_ERR_CUDA;
 
   li::AttnParams ap;
   std::memset(&ap, 0, sizeof(ap));
   ap.tl = dv.tl;
   ap.B = p->B; ap.H = p->H; ap.Lq = p->Lq; ap.T_f = p->frame_tokens; ap.n_cur = p->n_cur_frames;
-  ap.Nqb = dv.Nqb; ap.Nc = dv.Nc; ap.kmax = kmax; ap.has_box_full = has_full;
+  ap.Nqb = dv.Nqb; ap.Nc = dv.Nc; ap.kmax = kmax; ap.has_box_full = has_full; ap.Lt = p->Lt;
   const float scale = p->softmax_scale != 0.f ? p->softmax_scale : 1.0f / std::sqrt((float)p->d);
   ap.scale_log2 = scale * 1.4426950408889634f;
   ap.frame_idx = p->frame_idx; ap.sel_idx = sel_idx; ap.sel_cnt = sel_cnt;
   ap.o = (uint16_t *)o; ap.lse = lse_opt;
   int64_t n = 0;
-  const int e = li::launch_attn(ap, dv.meta, p->d, blk, tm_q, tm_kf, tm_k8, tm_vf, tm_v8, (cudaStream_t)cuda_stream, &n);
+  const int e = li::launch_attn(ap, dv.meta, p->d, blk, tm_q, tm_tk, tm_tv, tm_kf, tm_k8, tm_vf, tm_v8, (cudaStream_t)cuda_stream, &n);
   g_launches += n;
   if (e != 0 && std::getenv("LI_DEBUG") != nullptr)
     std::fprintf(stderr, "li_sparse_attn: CUDA error %d: %s\n", e, cudaGetErrorString((cudaError_t)e));

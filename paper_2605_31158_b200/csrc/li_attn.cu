@@ -65,6 +65,7 @@ enum {
 template <int D, int BLK, bool K3D>
 __global__ void __launch_bounds__(192, 2)
 li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_constant__ CUtensorMap tm_q,
+                      const __grid_constant__ CUtensorMap tm_tk, const __grid_constant__ CUtensorMap tm_tv,
                       const __grid_constant__ CUtensorMap tm_k_full, const __grid_constant__ CUtensorMap tm_k_8,
                       const __grid_constant__ CUtensorMap tm_v_full, const __grid_constant__ CUtensorMap tm_v_8) {
   using L = AttnSmem<D, BLK>;
@@ -97,6 +98,8 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
   const int M = tl.num_blocks(n_hist, p.T_f, BLK);
   const int Nc = tl.num_blocks(p.n_cur, p.T_f, BLK);
   const int n_qf = p.Lq / p.T_f;                       // query frames (3-D)
+  const int Nt = (p.Lt + BLK - 1) / BLK;               // text tiles (T of Eq. 11): dense, attended first, 1-D
+  const int tail_text = p.Lt - (Nt - 1) * BLK;
   const int64_t row_id = ((int64_t)b * p.H + h) * p.Nqb + i;
   const int valid_q = min(BLK, p.Lq - i * BLK);
   const int tail_cur = L_cur - (Nc - 1) * BLK, tail_hist = L_hist - (M - 1) * BLK;
@@ -108,6 +111,8 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
     tma_prefetch_desc(&tm_v_full);
     tma_prefetch_desc(&tm_k_8);
     tma_prefetch_desc(&tm_v_8);
+    tma_prefetch_desc(&tm_tk);
+    tma_prefetch_desc(&tm_tv);
     for (int k = 0; k < BAR_COUNT; ++k) mbar_init(bar(k), (k == BAR_P_FULL || k == BAR_P_FULL + 1) ? 4 : 1);
     *sT = 0;
     mbar_fence_init();
@@ -120,7 +125,7 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
   asm volatile("griddepcontrol.wait;" ::: "memory");     // sel_idx / sel_cnt come from li_block_select (PDL)
   const int cnt = p.sel_cnt[row_id];
   const int32_t *sel_row = p.sel_idx + row_id * p.kmax;
-  const int n_tiles = Nc + cnt;
+  const int n_tiles = Nt + Nc + cnt;                   // attended tiles: text | chunk | selected history
   for (int t = threadIdx.x; t < cnt && t < kSelCap; t += blockDim.x) sSel[t] = sel_row[t];
   // the frame list is read by the TMA producer for every half-tile: a global load there (L2 latency) would pace the
   // whole pipeline, so it is staged in shared memory once
@@ -137,31 +142,36 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
   // ascending) can only be the last selected one.  3-D: tiles of a region's last temporal group may hold fewer than
   // bt frames, border tiles fewer than bh grid rows.
   const int j_tail_hist = (cnt > 0 && sel_at(cnt - 1) == M - 1) ? n_tiles - 1 : -1;
-  auto tile_valid = [&](int j) -> int { return j == Nc - 1 ? tail_cur : (j == j_tail_hist ? tail_hist : BLK); };
-  auto tile_blk = [&](int j) -> int { return j < Nc ? j : sel_at(j - Nc); };
+  auto tile_valid = [&](int j) -> int {                // 1-D tiles (and text tiles in both modes): valid prefix
+    if (j < Nt) return j == Nt - 1 ? tail_text : BLK;
+    return j == Nt + Nc - 1 ? tail_cur : (j == j_tail_hist ? tail_hist : BLK);
+  };
+  auto tile_blk = [&](int j) -> int { return j < Nt + Nc ? j - Nt : sel_at(j - Nt - Nc); };   // block index in its region
   auto tile_info = [&](int j) -> int {                 // 3-D: (frames of tile j that exist) | (valid rows per slice) << 8
     const int blk = tile_blk(j);
-    const int nf = min(tl.bt, (j < Nc ? p.n_cur : n_hist) - (blk / per) * tl.bt);
+    const int nf = min(tl.bt, (j < Nt + Nc ? p.n_cur : n_hist) - (blk / per) * tl.bt);
     return nf | (min(tl.bh, tl.gh - ((blk % per) / tl.Wb) * tl.bh) * tl.bw) << 8;
   };
-  auto tile_info_cached = [&](int j) -> int { return j < kInfoCap ? (int)sInfo[j] : tile_info(j); };
+  auto tile_info_cached = [&](int j) -> int { return j - Nt < kInfoCap ? (int)sInfo[j - Nt] : tile_info(j); };
   auto tile_frames = [&](int j) -> int { return tile_info_cached(j) & 0xff; };
   auto halves = [&](int j) -> int {                    // half-tiles of tile j with at least one valid key
-    return k3d ? (tile_frames(j) > SPH ? 2 : 1) : (tile_valid(j) > HALF ? 2 : 1);
+    return (k3d && j >= Nt) ? (tile_frames(j) > SPH ? 2 : 1) : (tile_valid(j) > HALF ? 2 : 1);
   };
   // number of half-tiles with at least one valid key (a half-tile without any is skipped by every role)
   int T = 2 * n_tiles;
   if (k3d) {
     int part = 0;
     for (int j = threadIdx.x; j < n_tiles; j += blockDim.x) {
+      if (j < Nt) { part += tile_valid(j) > HALF ? 2 : 1; continue; }
       const int info = tile_info(j);                   // integer divisions once per tile, not once per half-tile per role
-      if (j < kInfoCap) sInfo[j] = (uint16_t)info;
+      if (j - Nt < kInfoCap) sInfo[j - Nt] = (uint16_t)info;
       part += (info & 0xff) > SPH ? 2 : 1;
     }
     if (part) atomicAdd(sT, part);
     __syncthreads();
     T = *sT;
   } else {
+    if (Nt > 0 && tail_text <= HALF) --T;
     if (Nc > 0 && tail_cur <= HALF) --T;
     if (j_tail_hist >= 0 && tail_hist <= HALF) --T;
   }
@@ -198,12 +208,24 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
       __syncwarp();
       int n = 0;                                     // running load index: slot = n % 4
       // loads HALF rows [t0, t0+HALF) of a region (history or chunk) into ring slot n % 4
-      auto load_half = [&](const CUtensorMap *tm_full, const CUtensorMap *tm_8, int j, int hh) {
-        const bool is_cur = j < Nc;
-        const int blk = is_cur ? j : sel_at(j - Nc);
+      auto load_half = [&](const CUtensorMap *tm_full, const CUtensorMap *tm_8, const CUtensorMap *tm_text, int j, int hh) {
+        const bool is_cur = j < Nt + Nc;
+        const int blk = tile_blk(j);
         const int f0 = is_cur ? n_hist : 0;            // first frame of the region inside this call's frame list
         const int slot = n & (kStages - 1);
         const uint32_t dst = sRing + slot * L::kStage, mb = bar(BAR_FULL + slot);
+        if (j < Nt) {
+          // text tile (T of Eq. 11): dense [B,H,Lt,d] tensor, rows past Lt are zero-filled by the hardware
+          mbar_wait(bar(BAR_EMPTY + slot), ((n >> 2) & 1) ^ 1);
+          if (elect_one()) {
+            mbar_arrive_expect_tx(mb, HALF * D * 2);
+#pragma unroll
+            for (int c = 0; c < D / 64; ++c) tma_load_4d(dst + c * L::kKVChunk, tm_text, mb, c * 64, j * BLK + hh * HALF, h, b);
+          }
+          __syncwarp();
+          ++n;
+          return;
+        }
         if (k3d) {
           // 3-D block (tg, hb, wb): the half-tile is SPH frame slices of 32 rows (bh grid rows x bw columns), each one
           // 5-D box (64 channels, bw, bh, head, page); grid rows >= grid_h are zero-filled by the hardware ("masked
@@ -272,11 +294,11 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
 
       // load order == consumption order of the MMA warp: K0 K1 | V0 K2 | V1 K3 | ...
       int kj = 0, kh = 0, vj = 0, vh = 0;
-      load_half(&tm_k_full, &tm_k_8, kj, kh); advance(kj, kh);
-      if (T > 1) { load_half(&tm_k_full, &tm_k_8, kj, kh); advance(kj, kh); }
+      load_half(&tm_k_full, &tm_k_8, &tm_tk, kj, kh); advance(kj, kh);
+      if (T > 1) { load_half(&tm_k_full, &tm_k_8, &tm_tk, kj, kh); advance(kj, kh); }
       for (int t = 0; t < T; ++t) {
-        load_half(&tm_v_full, &tm_v_8, vj, vh); advance(vj, vh);
-        if (t + 2 < T) { load_half(&tm_k_full, &tm_k_8, kj, kh); advance(kj, kh); }
+        load_half(&tm_v_full, &tm_v_8, &tm_tv, vj, vh); advance(vj, vh);
+        if (t + 2 < T) { load_half(&tm_k_full, &tm_k_8, &tm_tk, kj, kh); advance(kj, kh); }
       }
     } else if (warp == 5) {
       // =============================== MMA issuer ===============================
@@ -340,7 +362,7 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
         // the rest is padding): 1-D blocks have one valid prefix; a 3-D slice is one frame's bh x bw patch, whose
         // grid rows beyond grid_h (and whose frame, beyond the region) are padding
         int vs[SPH];
-        if (k3d) {
+        if (k3d && j >= Nt) {
           const int info = tile_info_cached(j), nf = info & 0xff, vrow = info >> 8;
 #pragma unroll
           for (int s_ = 0; s_ < SPH; ++s_) vs[s_] = (hh * SPH + s_ < nf) ? vrow : 0;
@@ -476,7 +498,8 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
 }
 
 template <int D, int BLK, bool K3D>
-static int launch_one(const AttnParams &ap, const BatchMeta &meta, const CUtensorMap &tm_q, const CUtensorMap &tm_k_full,
+static int launch_one(const AttnParams &ap, const BatchMeta &meta, const CUtensorMap &tm_q, const CUtensorMap &tm_tk,
+                      const CUtensorMap &tm_tv, const CUtensorMap &tm_k_full,
                       const CUtensorMap &tm_k_8, const CUtensorMap &tm_v_full, const CUtensorMap &tm_v_8,
                       cudaStream_t st) {
   auto kern = li_sparse_attn_kernel<D, BLK, K3D>;
@@ -493,19 +516,19 @@ static int launch_one(const AttnParams &ap, const BatchMeta &meta, const CUtenso
   cfg.stream = st;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  e = cudaLaunchKernelEx(&cfg, kern, ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8);
+  e = cudaLaunchKernelEx(&cfg, kern, ap, meta, tm_q, tm_tk, tm_tv, tm_k_full, tm_k_8, tm_v_full, tm_v_8);
   if (e != cudaSuccess) return (int)e;
   return (int)cudaGetLastError();
 }
 
 int launch_attn(const AttnParams &ap, const BatchMeta &meta, int d, int blk, const CUtensorMap &tm_q,
-                const CUtensorMap &tm_k_full, const CUtensorMap &tm_k_8, const CUtensorMap &tm_v_full,
+                const CUtensorMap &tm_tk, const CUtensorMap &tm_tv, const CUtensorMap &tm_k_full, const CUtensorMap &tm_k_8, const CUtensorMap &tm_v_full,
                 const CUtensorMap &tm_v_8, cudaStream_t st, int64_t *n_launches) {
   int e;
   const bool k3 = ap.tl.bt > 0;
 #define LI_LAUNCH(DD, BB)                                                                                  \
-  (k3 ? launch_one<DD, BB, true>(ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st)                \
-      : launch_one<DD, BB, false>(ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st))
+  (k3 ? launch_one<DD, BB, true>(ap, meta, tm_q, tm_tk, tm_tv, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st)                \
+      : launch_one<DD, BB, false>(ap, meta, tm_q, tm_tk, tm_tv, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st))
   if (d == 128 && blk == 128) e = LI_LAUNCH(128, 128);
   else if (d == 128 && blk == 64) e = LI_LAUNCH(128, 64);
   else if (d == 64 && blk == 128) e = LI_LAUNCH(64, 128);

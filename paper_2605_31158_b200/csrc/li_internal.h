@@ -44,6 +44,7 @@ struct SelectParams {
 struct AttnParams {
   Tiling tl;
   int32_t B, H, Lq, T_f, n_cur, Nqb, Nc, kmax;
+  int32_t Lt;             // text tokens (T of Eq. 11), 0 = none
   int32_t has_box_full;   // 1: tensor maps with a full-block box exist (T_f >= block)
   float scale_log2;       // softmax_scale * log2(e)
   const int32_t *frame_idx;
@@ -56,7 +57,7 @@ struct AttnParams {
 // launches (defined in the .cu files); return cudaError_t as int
 int launch_select(const SelectParams &sp, const BatchMeta &meta, cudaStream_t st, int64_t *n_launches);
 int launch_attn(const AttnParams &ap, const BatchMeta &meta, int d, int blk, const CUtensorMap &tm_q,
-                const CUtensorMap &tm_k_full, const CUtensorMap &tm_k_8, const CUtensorMap &tm_v_full,
+                const CUtensorMap &tm_tk, const CUtensorMap &tm_tv, const CUtensorMap &tm_k_full, const CUtensorMap &tm_k_8, const CUtensorMap &tm_v_full,
                 const CUtensorMap &tm_v_8, cudaStream_t st, int64_t *n_launches);
 
 }  // namespace li

@@ -127,6 +127,15 @@ def test_3d_tiling_validation(L):
             assert L.li_sparse_attn(ctypes.byref(pb), 0x60000, 0x70000, 8, 0x80000, None, None, 0, None) == code, bad
 
 
+def test_text_prefix_validation(L):
+    p, fo = make_problem(Lt=77, text_k=0x90000, text_v=0xA0000, t_sb=2 * 77 * 64, t_sh=77 * 64, t_st=64)
+    assert L.li_workspace_bytes(ctypes.byref(p), 8) > 0
+    for bad in (dict(text_k=0), dict(text_v=0x90008), dict(t_st=60), dict(t_sh=0), dict(Lt=-1)):
+        pb, keep = make_problem(**{**dict(Lt=77, text_k=0x90000, text_v=0xA0000, t_sb=2 * 77 * 64, t_sh=77 * 64, t_st=64), **bad})
+        assert L.li_workspace_bytes(ctypes.byref(pb), 8) == 0, bad
+        assert L.li_sparse_attn(ctypes.byref(pb), 0x60000, 0x70000, 8, 0x80000, None, None, 0, None) == li.LI_ERR_INVALID_ARG, bad
+
+
 def test_binding_refuses_cpu_tensors():
     import torch
     q = torch.zeros((1, 2, 256, 64), dtype=torch.bfloat16)

@@ -61,3 +61,44 @@ def test_3d_dense_and_chunk_only(P):
         ref = torch.nn.functional.scaled_dot_product_attention(prob.q[0].float(), K, V)
         diff = (buf.o[0].float().cpu() - ref).abs()
         assert torch.isfinite(buf.o.float()).all() and diff.max() <= P.MAX_ABS and diff.mean() <= P.MEAN_ABS
+
+
+@pytest.mark.parametrize("mode,Lt", [("1d", 77), ("1d", 40), ("1d", 256), ("3d", 77), ("3d", 136)])
+def test_text_prefix_is_always_attended(P, mode, Lt):
+    """T of Eq. 11: a dense text K/V region attended by every query block on top of the chunk and
+    the selected history; ragged text tail, text shorter than one half-tile, strided text tensor."""
+    import paper_2605_31158_b200 as li
+    from oracle import li_oracle as O
+    if mode == "1d":
+        spec = W.spec_small(name="text-1d", H=2, d=128, block=128, frame_tokens=200, n_cur_frames=2, n_pages=10,
+                            n_mem=(2,), n_win=(2,), density=Fraction(1, 2))
+    else:
+        spec = small3d("text-3d", (10, 16), (4, 8, 4), 4, (2,), (3,))
+    prob = W.build(spec)
+    g = torch.Generator().manual_seed(1000 + Lt)
+    wide = torch.randn((1, spec.H, Lt, 2 * spec.d), generator=g).to(torch.bfloat16)       # [..., :d] = K, [..., d:] = V
+    tk, tv = wide[..., :spec.d], wide[..., spec.d:]                                        # token stride 2d
+    dev = "cuda:0"
+    wide_d = wide.to(dev)
+    ctx = li.Context(prob.q.to(dev), prob.k_cache.to(dev), prob.v_cache.to(dev), torch.from_numpy(prob.frame_idx).to(dev),
+                     prob.frame_off, spec.n_cur_frames, spec.block, grid=spec.grid, block3d=spec.block3d,
+                     text_k=wide_d[..., :spec.d], text_v=wide_d[..., spec.d:])
+    buf = li.Buffers(ctx, prob.kmax, want_scores=True)
+    buf.o.fill_(float("nan"))
+    li.forward(ctx, prob.top_k, buf)
+    torch.cuda.synchronize()
+    osel, osc = P.oracle_select(prob)                      # text takes no part in pooling / selection
+    P.check_selection(prob, buf, osel, osc)
+    gsel = [g_[0] for g_ in P.gpu_selection(prob, buf)]
+    u16 = lambda t: t.contiguous().view(torch.int16).numpy().view(np.uint16)
+    s = spec
+    if s.block3d is not None:
+        o_ref, lse_ref = O.sparse_attn_3d(prob.u16(prob.q), prob.u16(prob.k_cache), prob.u16(prob.v_cache), prob.frame_idx,
+                                          prob.frame_off, s.n_cur_frames, *s.grid, *s.block3d, gsel,
+                                          text_k=u16(tk), text_v=u16(tv))
+    else:
+        o_ref, lse_ref = O.sparse_attn(prob.u16(prob.q), prob.u16(prob.k_cache), prob.u16(prob.v_cache), prob.frame_idx,
+                                       prob.frame_off, s.n_cur_frames, s.block, s.block, gsel,
+                                       text_k=u16(tk), text_v=u16(tv))
+    mx, mean = P.compare_output(buf.o, buf.lse, o_ref, lse_ref)
+    print(f"text {mode} Lt={Lt}: max-abs {mx:.3g} mean-abs {mean:.3g}")
