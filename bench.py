@@ -300,6 +300,16 @@ def run_cuda(args):
                 ts.append(a.elapsed_time(b_))
             return float(np.mean(ts[2:]))
         extras["attn_ms_l2_warm"] = time_attn(ctx, flush_l2=False)
+        ts = []
+        for _ in range(12):                              # select with the pooled history keys reused (denoising steps 2..K)
+            flush.fill_(5)
+            a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            li.li_block_select(ctx, prob.top_k, buf.kmax, buf.sel_idx, buf.sel_cnt, buf.workspace, None, stream, reuse_kbar=True)
+            b_.record(stream)
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b_))
+        extras["select_ms_reuse_kbar"] = float(np.mean(ts[2:]))
         order = torch.from_numpy(prob.frame_idx.astype(np.int64)).to(dev)
         free_b = torch.cuda.mem_get_info()[0]
         need_b = 2 * order.numel() * kc[0].numel() * 2

@@ -94,6 +94,15 @@ int li_block_select(const li_problem *p, const int32_t *top_k_host, int32_t kmax
                     int32_t *sel_idx, int32_t *sel_cnt, float *scores_opt, int32_t score_pitch,
                     void *workspace, size_t workspace_bytes, void *cuda_stream);
 
+/* Same as li_block_select, but the pooled historical keys kbar are NOT recomputed: `workspace` must still hold them
+ * from an earlier li_block_select on the same history (same frame lists, same K pages, same tiling).  Within one
+ * chunk the historical K of a layer does not change across the K denoising steps (the context
+ * is reconstructed once per chunk), so only Q has to be pooled again: the call reads Lq*d*2*H bytes instead of
+ * (Lq + L_hist)*d*2*H. */
+int li_block_select_reuse_kbar(const li_problem *p, const int32_t *top_k_host, int32_t kmax,
+                               int32_t *sel_idx, int32_t *sel_cnt, float *scores_opt, int32_t score_pitch,
+                               void *workspace, size_t workspace_bytes, void *cuda_stream);
+
 /* Eq. 11 + attention.  Query block i of (b,h) attends ALL text tokens (if any), ALL chunk tokens
  * (bidirectional inside the chunk) plus the valid tokens of historical blocks sel_idx[b,h,i,0..sel_cnt[b,h,i]); the same
  * indices address K and V.  softmax in fp32 (online), bf16 tcgen05 MMAs with fp32 accumulation.

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libli.so")
 LI_OK, LI_ERR_INVALID_ARG, LI_ERR_UNSUPPORTED, LI_ERR_WORKSPACE, LI_ERR_CUDA = 0, -1, -2, -3, -4
 LI_MAX_CALLS = 64
 
-EXPORTS = ("li_block_select", "li_sparse_attn", "li_workspace_bytes", "li_launch_count",
+EXPORTS = ("li_block_select", "li_block_select_reuse_kbar", "li_sparse_attn", "li_workspace_bytes", "li_launch_count",
            "li_reset_launch_count", "li_strerror", "li_version")
 
 
@@ -65,6 +65,8 @@ def lib() -> ctypes.CDLL:
         L.li_block_select.argtypes = [P, ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p, ctypes.c_void_p,
                                       ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p, ctypes.c_size_t,
                                       ctypes.c_void_p]
+        L.li_block_select_reuse_kbar.restype = ctypes.c_int
+        L.li_block_select_reuse_kbar.argtypes = L.li_block_select.argtypes
         L.li_sparse_attn.restype = ctypes.c_int
         L.li_sparse_attn.argtypes = [P, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p,
                                      ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p]
@@ -166,14 +168,15 @@ def li_workspace_bytes(ctx: Context, kmax: int) -> int:
 
 def li_block_select(ctx: Context, top_k: Sequence[int], kmax: int, sel_idx: torch.Tensor, sel_cnt: torch.Tensor,
                     workspace: torch.Tensor, scores: Optional[torch.Tensor] = None,
-                    stream: Optional[torch.cuda.Stream] = None) -> None:
-    """li_block_select (include/li.h).  sel_idx int32 [B,H,Nqb,kmax], sel_cnt int32 [B,H,Nqb],
+                    stream: Optional[torch.cuda.Stream] = None, reuse_kbar: bool = False) -> None:
+    """li_block_select / li_block_select_reuse_kbar (include/li.h).  sel_idx int32 [B,H,Nqb,kmax], sel_cnt int32 [B,H,Nqb],
     scores None or fp32 [B,H,Nqb,pitch]; workspace: uint8 CUDA tensor of >= li_workspace_bytes."""
     tk = np.ascontiguousarray(np.asarray(top_k, dtype=np.int32))
     if len(tk) != ctx.B:
         raise ValueError("top_k must have B entries")
     pitch = int(scores.shape[-1]) if scores is not None else 0
-    rc = lib().li_block_select(ctypes.byref(ctx.p), tk.ctypes.data, int(kmax), sel_idx.data_ptr(),
+    fn = lib().li_block_select_reuse_kbar if reuse_kbar else lib().li_block_select
+    rc = fn(ctypes.byref(ctx.p), tk.ctypes.data, int(kmax), sel_idx.data_ptr(),
                                sel_cnt.data_ptr(), scores.data_ptr() if scores is not None else None, pitch,
                                workspace.data_ptr(), workspace.numel() * workspace.element_size(),
                                _stream_ptr(stream))

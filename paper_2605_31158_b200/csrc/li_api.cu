@@ -147,9 +147,9 @@ size_t li_workspace_bytes(const li_problem *p, int32_t kmax) {
   return ws_bytes(p, dv);
 }
 
-int li_block_select(const li_problem *p, const int32_t *top_k_host, int32_t kmax, int32_t *sel_idx, int32_t *sel_cnt,
-                    float *scores_opt, int32_t score_pitch, void *workspace, size_t workspace_bytes,
-                    void *cuda_stream) {
+static int block_select_impl(const li_problem *p, const int32_t *top_k_host, int32_t kmax, int32_t *sel_idx,
+                             int32_t *sel_cnt, float *scores_opt, int32_t score_pitch, void *workspace,
+                             size_t workspace_bytes, void *cuda_stream, int skip_k) {
   Derived dv;
   int rc = check_problem(p, &dv);
   if (rc != LI_OK) return rc;
@@ -168,6 +168,7 @@ int li_block_select(const li_problem *p, const int32_t *top_k_host, int32_t kmax
   li::SelectParams sp;
   std::memset(&sp, 0, sizeof(sp));
   sp.tl = dv.tl;
+  sp.skip_k = skip_k;
   sp.B = p->B; sp.H = p->H; sp.Lq = p->Lq; sp.d = p->d; sp.T_f = p->frame_tokens; sp.blk = p->block_k;
   sp.n_cur = p->n_cur_frames; sp.Nqb = dv.Nqb; sp.Mmax = dv.Mmax; sp.kmax = kmax;
   sp.score_pitch = score_pitch;
@@ -184,6 +185,20 @@ int li_block_select(const li_problem *p, const int32_t *top_k_host, int32_t kmax
   const int e = li::launch_select(sp, dv.meta, (cudaStream_t)cuda_stream, &n);
   g_launches += n;
   return e == 0 ? LI_OK : LI_ERR_CUDA;
+}
+
+int li_block_select(const li_problem *p, const int32_t *top_k_host, int32_t kmax, int32_t *sel_idx, int32_t *sel_cnt,
+                    float *scores_opt, int32_t score_pitch, void *workspace, size_t workspace_bytes,
+                    void *cuda_stream) {
+  return block_select_impl(p, top_k_host, kmax, sel_idx, sel_cnt, scores_opt, score_pitch, workspace, workspace_bytes,
+                           cuda_stream, 0);
+}
+
+int li_block_select_reuse_kbar(const li_problem *p, const int32_t *top_k_host, int32_t kmax, int32_t *sel_idx,
+                               int32_t *sel_cnt, float *scores_opt, int32_t score_pitch, void *workspace,
+                               size_t workspace_bytes, void *cuda_stream) {
+  return block_select_impl(p, top_k_host, kmax, sel_idx, sel_cnt, scores_opt, score_pitch, workspace, workspace_bytes,
+                           cuda_stream, 1);
 }
 
 int li_sparse_attn(const li_problem *p, const int32_t *sel_idx, const int32_t *sel_cnt, int32_t kmax, void *o,

@@ -62,12 +62,11 @@ enum {
   BAR_COUNT
 };
 
-template <int D, int BLK, bool K3D>
-__global__ void __launch_bounds__(192, 2)
-li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_constant__ CUtensorMap tm_q,
-                      const __grid_constant__ CUtensorMap tm_tk, const __grid_constant__ CUtensorMap tm_tv,
-                      const __grid_constant__ CUtensorMap tm_k_full, const __grid_constant__ CUtensorMap tm_k_8,
-                      const __grid_constant__ CUtensorMap tm_v_full, const __grid_constant__ CUtensorMap tm_v_8) {
+template <int D, int BLK, bool K3D, bool TEXT>
+__device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &meta, const CUtensorMap &tm_q,
+                                          const CUtensorMap &tm_k_full, const CUtensorMap &tm_k_8,
+                                          const CUtensorMap &tm_v_full, const CUtensorMap &tm_v_8,
+                                          const CUtensorMap &tm_tk, const CUtensorMap &tm_tv) {
   using L = AttnSmem<D, BLK>;
   constexpr int HALF = L::HALF;
   extern __shared__ uint8_t smem_raw[];
@@ -98,7 +97,7 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
   const int M = tl.num_blocks(n_hist, p.T_f, BLK);
   const int Nc = tl.num_blocks(p.n_cur, p.T_f, BLK);
   const int n_qf = p.Lq / p.T_f;                       // query frames (3-D)
-  const int Nt = (p.Lt + BLK - 1) / BLK;               // text tiles (T of Eq. 11): dense, attended first, 1-D
+  const int Nt = TEXT ? (p.Lt + BLK - 1) / BLK : 0;    // text tiles (T of Eq. 11): dense, attended first, 1-D
   const int tail_text = p.Lt - (Nt - 1) * BLK;
   const int64_t row_id = ((int64_t)b * p.H + h) * p.Nqb + i;
   const int valid_q = min(BLK, p.Lq - i * BLK);
@@ -111,8 +110,10 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
     tma_prefetch_desc(&tm_v_full);
     tma_prefetch_desc(&tm_k_8);
     tma_prefetch_desc(&tm_v_8);
-    tma_prefetch_desc(&tm_tk);
-    tma_prefetch_desc(&tm_tv);
+    if (TEXT) {
+      tma_prefetch_desc(&tm_tk);
+      tma_prefetch_desc(&tm_tv);
+    }
     for (int k = 0; k < BAR_COUNT; ++k) mbar_init(bar(k), (k == BAR_P_FULL || k == BAR_P_FULL + 1) ? 4 : 1);
     *sT = 0;
     mbar_fence_init();
@@ -143,7 +144,7 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
   // bt frames, border tiles fewer than bh grid rows.
   const int j_tail_hist = (cnt > 0 && sel_at(cnt - 1) == M - 1) ? n_tiles - 1 : -1;
   auto tile_valid = [&](int j) -> int {                // 1-D tiles (and text tiles in both modes): valid prefix
-    if (j < Nt) return j == Nt - 1 ? tail_text : BLK;
+    if (TEXT && j < Nt) return j == Nt - 1 ? tail_text : BLK;
     return j == Nt + Nc - 1 ? tail_cur : (j == j_tail_hist ? tail_hist : BLK);
   };
   auto tile_blk = [&](int j) -> int { return j < Nt + Nc ? j - Nt : sel_at(j - Nt - Nc); };   // block index in its region
@@ -155,14 +156,14 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
   auto tile_info_cached = [&](int j) -> int { return j - Nt < kInfoCap ? (int)sInfo[j - Nt] : tile_info(j); };
   auto tile_frames = [&](int j) -> int { return tile_info_cached(j) & 0xff; };
   auto halves = [&](int j) -> int {                    // half-tiles of tile j with at least one valid key
-    return (k3d && j >= Nt) ? (tile_frames(j) > SPH ? 2 : 1) : (tile_valid(j) > HALF ? 2 : 1);
+    return (k3d && (!TEXT || j >= Nt)) ? (tile_frames(j) > SPH ? 2 : 1) : (tile_valid(j) > HALF ? 2 : 1);
   };
   // number of half-tiles with at least one valid key (a half-tile without any is skipped by every role)
   int T = 2 * n_tiles;
   if (k3d) {
     int part = 0;
     for (int j = threadIdx.x; j < n_tiles; j += blockDim.x) {
-      if (j < Nt) { part += tile_valid(j) > HALF ? 2 : 1; continue; }
+      if (TEXT && j < Nt) { part += tile_valid(j) > HALF ? 2 : 1; continue; }
       const int info = tile_info(j);                   // integer divisions once per tile, not once per half-tile per role
       if (j - Nt < kInfoCap) sInfo[j - Nt] = (uint16_t)info;
       part += (info & 0xff) > SPH ? 2 : 1;
@@ -171,7 +172,7 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
     __syncthreads();
     T = *sT;
   } else {
-    if (Nt > 0 && tail_text <= HALF) --T;
+    if (TEXT && Nt > 0 && tail_text <= HALF) --T;
     if (Nc > 0 && tail_cur <= HALF) --T;
     if (j_tail_hist >= 0 && tail_hist <= HALF) --T;
   }
@@ -214,7 +215,7 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
         const int f0 = is_cur ? n_hist : 0;            // first frame of the region inside this call's frame list
         const int slot = n & (kStages - 1);
         const uint32_t dst = sRing + slot * L::kStage, mb = bar(BAR_FULL + slot);
-        if (j < Nt) {
+        if (TEXT && j < Nt) {
           // text tile (T of Eq. 11): dense [B,H,Lt,d] tensor, rows past Lt are zero-filled by the hardware
           mbar_wait(bar(BAR_EMPTY + slot), ((n >> 2) & 1) ^ 1);
           if (elect_one()) {
@@ -362,7 +363,7 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
         // the rest is padding): 1-D blocks have one valid prefix; a 3-D slice is one frame's bh x bw patch, whose
         // grid rows beyond grid_h (and whose frame, beyond the region) are padding
         int vs[SPH];
-        if (k3d && j >= Nt) {
+        if (k3d && (!TEXT || j >= Nt)) {
           const int info = tile_info_cached(j), nf = info & 0xff, vrow = info >> 8;
 #pragma unroll
           for (int s_ = 0; s_ < SPH; ++s_) vs[s_] = (hh * SPH + s_ < nf) ? vrow : 0;
@@ -497,14 +498,34 @@ li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_con
   if (warp == 5) tmem_dealloc(tmem, kTmemCols);
 }
 
+// Two entry points: the text maps are kernel parameters only of the variant that attends a text prefix (adding two
+// unused 128-byte tensor maps to the parameter block of the plain kernel measurably slowed it down).
 template <int D, int BLK, bool K3D>
+__global__ void __launch_bounds__(192, 2)
+li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_constant__ CUtensorMap tm_q,
+                      const __grid_constant__ CUtensorMap tm_k_full, const __grid_constant__ CUtensorMap tm_k_8,
+                      const __grid_constant__ CUtensorMap tm_v_full, const __grid_constant__ CUtensorMap tm_v_8) {
+  attn_body<D, BLK, K3D, false>(p, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, tm_q, tm_q);
+}
+
+template <int D, int BLK, bool K3D>
+__global__ void __launch_bounds__(192, 2)
+li_sparse_attn_text_kernel(const AttnParams p, const BatchMeta meta, const __grid_constant__ CUtensorMap tm_q,
+                           const __grid_constant__ CUtensorMap tm_k_full, const __grid_constant__ CUtensorMap tm_k_8,
+                           const __grid_constant__ CUtensorMap tm_v_full, const __grid_constant__ CUtensorMap tm_v_8,
+                           const __grid_constant__ CUtensorMap tm_tk, const __grid_constant__ CUtensorMap tm_tv) {
+  attn_body<D, BLK, K3D, true>(p, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, tm_tk, tm_tv);
+}
+
+template <int D, int BLK, bool K3D, bool TEXT>
 static int launch_one(const AttnParams &ap, const BatchMeta &meta, const CUtensorMap &tm_q, const CUtensorMap &tm_tk,
                       const CUtensorMap &tm_tv, const CUtensorMap &tm_k_full,
                       const CUtensorMap &tm_k_8, const CUtensorMap &tm_v_full, const CUtensorMap &tm_v_8,
                       cudaStream_t st) {
-  auto kern = li_sparse_attn_kernel<D, BLK, K3D>;
   constexpr int smem = AttnSmem<D, BLK>::kTotal;
-  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  cudaError_t e;
+  if constexpr (TEXT) e = cudaFuncSetAttribute(li_sparse_attn_text_kernel<D, BLK, K3D>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  else e = cudaFuncSetAttribute(li_sparse_attn_kernel<D, BLK, K3D>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   if (e != cudaSuccess) return (int)e;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
@@ -516,7 +537,10 @@ static int launch_one(const AttnParams &ap, const BatchMeta &meta, const CUtenso
   cfg.stream = st;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  e = cudaLaunchKernelEx(&cfg, kern, ap, meta, tm_q, tm_tk, tm_tv, tm_k_full, tm_k_8, tm_v_full, tm_v_8);
+  if constexpr (TEXT)
+    e = cudaLaunchKernelEx(&cfg, li_sparse_attn_text_kernel<D, BLK, K3D>, ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, tm_tk, tm_tv);
+  else
+    e = cudaLaunchKernelEx(&cfg, li_sparse_attn_kernel<D, BLK, K3D>, ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8);
   if (e != cudaSuccess) return (int)e;
   return (int)cudaGetLastError();
 }
@@ -526,14 +550,16 @@ int launch_attn(const AttnParams &ap, const BatchMeta &meta, int d, int blk, con
                 const CUtensorMap &tm_v_8, cudaStream_t st, int64_t *n_launches) {
   int e;
   const bool k3 = ap.tl.bt > 0;
-#define LI_LAUNCH(DD, BB)                                                                                  \
-  (k3 ? launch_one<DD, BB, true>(ap, meta, tm_q, tm_tk, tm_tv, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st)                \
-      : launch_one<DD, BB, false>(ap, meta, tm_q, tm_tk, tm_tv, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st))
+#define LI_LAUNCH2(DD, BB, K3)                                                                               \
+  (ap.Lt > 0 ? launch_one<DD, BB, K3, true>(ap, meta, tm_q, tm_tk, tm_tv, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st)  \
+             : launch_one<DD, BB, K3, false>(ap, meta, tm_q, tm_tk, tm_tv, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st))
+#define LI_LAUNCH(DD, BB) (k3 ? LI_LAUNCH2(DD, BB, true) : LI_LAUNCH2(DD, BB, false))
   if (d == 128 && blk == 128) e = LI_LAUNCH(128, 128);
   else if (d == 128 && blk == 64) e = LI_LAUNCH(128, 64);
   else if (d == 64 && blk == 128) e = LI_LAUNCH(64, 128);
   else e = LI_LAUNCH(64, 64);
 #undef LI_LAUNCH
+#undef LI_LAUNCH2
   if (e == 0 && n_launches) *n_launches += 1;
   return e;
 }

@@ -26,6 +26,7 @@ struct Tiling {
 
 struct SelectParams {
   Tiling tl;
+  int32_t skip_k;   // 1: kbar in the workspace is still valid (li_block_select_reuse_kbar): pool Q only
   int32_t B, H, Lq, d, T_f, blk, n_cur, Nqb, Mmax, Mp, kmax, score_pitch;   // Mp = Mmax rounded up to 32
   const uint16_t *q;
   int64_t q_sb, q_sh, q_st;

@@ -306,7 +306,7 @@ __global__ void __launch_bounds__(kTopkWarps * 32) li_topk_kernel(const SelectPa
 
 int launch_select(const SelectParams &sp, const BatchMeta &meta, cudaStream_t st, int64_t *n_launches) {
   {
-    dim3 grid(sp.Nqb + sp.Mmax, sp.H, sp.B);
+    dim3 grid(sp.Nqb + (sp.skip_k ? 0 : sp.Mmax), sp.H, sp.B);
     if (sp.tl.bt > 0) {
       if (sp.d == 128) li_pool_kernel<128, true><<<grid, kPoolThreads, 0, st>>>(sp, meta);
       else li_pool_kernel<64, true><<<grid, kPoolThreads, 0, st>>>(sp, meta);

@@ -227,3 +227,23 @@ def test_batch_of_64_calls(P):
     assert prob.B == 64
     excused, mx, mean = P.full_parity(prob)
     print(f"small-b64: excused={excused} max-abs={mx:.3g} mean-abs={mean:.3g}")
+
+
+def test_select_reuse_kbar_across_denoising_steps(P):
+    """li_block_select_reuse_kbar: the history is static inside a chunk, only Q changes between denoising steps.
+    After one full select, a second select with a NEW Q and reuse must equal the oracle run on the new Q."""
+    import paper_2605_31158_b200 as li
+    spec = W.spec_small(name="small-reuse", H=2, d=128, block=128, frame_tokens=200, n_cur_frames=2, n_pages=10,
+                        n_mem=(2,), n_win=(3,), density=Fraction(1, 2))
+    prob = W.build(spec)
+    ctx = P.upload(prob)
+    buf = li.Buffers(ctx, prob.kmax, want_scores=True)
+    li.li_block_select(ctx, prob.top_k, buf.kmax, buf.sel_idx, buf.sel_cnt, buf.workspace, buf.scores)
+    g = torch.Generator().manual_seed(77)
+    prob.q = torch.randn(prob.q.shape, generator=g).to(torch.bfloat16)           # next denoising step: new queries
+    ctx.q.copy_(prob.q)
+    buf.sel_idx.fill_(-7)
+    li.li_block_select(ctx, prob.top_k, buf.kmax, buf.sel_idx, buf.sel_cnt, buf.workspace, buf.scores, reuse_kbar=True)
+    torch.cuda.synchronize()
+    osel, osc = P.oracle_select(prob)
+    P.check_selection(prob, buf, osel, osc)
