@@ -109,11 +109,16 @@ int li_block_select_reuse_kbar(const li_problem *p, const int32_t *top_k_host, i
  *   o       : bf16 [B,H,Lq,d], contiguous.
  *   lse_opt : NULL or fp32 [B,H,Lq]: log sum_n exp(scale * q.k_n) (natural log).
  * An empty context (no chunk and no selected block) gives o = 0, lse = -inf.
- * sel_idx values must lie in [0, M_b); they are not validated on the host. */
+ * sel_idx values must lie in [0, M_b); they are not validated on the host.
+ *   workspace : optional.  With >= li_workspace_bytes(p, kmax) bytes (256-byte aligned; the same buffer li_block_select
+ *               used: its pooled keys are left intact) the kernel may split the query blocks of a sparsely filled last
+ *               wave of CTAs across several CTAs and merge their partial results with a second, small launch
+ *               (results equal up to fp32 rounding of the merge).  NULL or a smaller buffer: never split. */
 int li_sparse_attn(const li_problem *p, const int32_t *sel_idx, const int32_t *sel_cnt, int32_t kmax,
                    void *o, float *lse_opt, void *workspace, size_t workspace_bytes, void *cuda_stream);
 
-/* Bytes of workspace both calls need for problem p (0 on invalid p). */
+/* Bytes of workspace the calls above need for problem p (0 on invalid p): li_block_select's pooled means and score keys,
+ * followed by the partial-result buffers of li_sparse_attn's split (a fixed ~21 MB at d = 128). */
 size_t li_workspace_bytes(const li_problem *p, int32_t kmax);
 
 /* Number of kernel launches the two calls above issued since the last li_reset_launch_count()

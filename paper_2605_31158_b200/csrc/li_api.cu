@@ -136,6 +136,10 @@ size_t ws_bytes(const li_problem *p, const Derived &dv) {
   return qbar + kbar + keys;
 }
 
+// partial results of the attention kernel's tail-wave split: [slots][128 rows][d] fp32 + [slots][128] float2
+size_t ws_split_o_bytes(const li_problem *p) { return align256((size_t)li::kMaxSplitSlots * 128 * p->d * 4); }
+size_t ws_split_bytes(const li_problem *p) { return ws_split_o_bytes(p) + align256((size_t)li::kMaxSplitSlots * 128 * 8); }
+
 }  // namespace
 
 extern "C" {
@@ -144,7 +148,7 @@ size_t li_workspace_bytes(const li_problem *p, int32_t kmax) {
   (void)kmax;
   Derived dv;
   if (check_problem(p, &dv) != LI_OK) return 0;
-  return ws_bytes(p, dv);
+  return ws_bytes(p, dv) + ws_split_bytes(p);
 }
 
 static int block_select_impl(const li_problem *p, const int32_t *top_k_host, int32_t kmax, int32_t *sel_idx,
@@ -155,7 +159,8 @@ static int block_select_impl(const li_problem *p, const int32_t *top_k_host, int
   if (rc != LI_OK) return rc;
   if (top_k_host == nullptr || sel_idx == nullptr || sel_cnt == nullptr || kmax < 1) return LI_ERR_INVALID_ARG;
   if (scores_opt != nullptr && score_pitch < dv.Mmax) return LI_ERR_INVALID_ARG;
-  if (workspace == nullptr || workspace_bytes < ws_bytes(p, dv) || ((uintptr_t)workspace & 255u)) return LI_ERR_WORKSPACE;
+  if (workspace == nullptr || workspace_bytes < ws_bytes(p, dv) + ws_split_bytes(p) || ((uintptr_t)workspace & 255u))
+    return LI_ERR_WORKSPACE;
   for (int b = 0; b < p->B; ++b) {
     if (top_k_host[b] < 0) return LI_ERR_INVALID_ARG;
     const int n_hist = dv.meta.frame_off[b + 1] - dv.meta.frame_off[b] - p->n_cur_frames;
@@ -203,12 +208,15 @@ int li_block_select_reuse_kbar(const li_problem *p, const int32_t *top_k_host, i
 
 int li_sparse_attn(const li_problem *p, const int32_t *sel_idx, const int32_t *sel_cnt, int32_t kmax, void *o,
                    float *lse_opt, void *workspace, size_t workspace_bytes, void *cuda_stream) {
-  (void)workspace; (void)workspace_bytes;   // the attention kernel needs no scratch memory
   Derived dv;
   int rc = check_problem(p, &dv);
   if (rc != LI_OK) return rc;
   if (sel_idx == nullptr || sel_cnt == nullptr || o == nullptr || kmax < 1) return LI_ERR_INVALID_ARG;
   if ((uintptr_t)o & 15u) return LI_ERR_INVALID_ARG;
+  if (workspace != nullptr && ((uintptr_t)workspace & 255u)) return LI_ERR_WORKSPACE;
+  // scratch is optional here: only the tail-wave split uses it (its region lies behind li_block_select's, so pooled
+  // keys kept for li_block_select_reuse_kbar survive); without a full-size workspace the split is simply not used
+  const bool have_ws = workspace != nullptr && workspace_bytes >= ws_bytes(p, dv) + ws_split_bytes(p);
 
   const int blk = p->block_k;
   const int half = blk / 2;                 // K/V are fetched as half-tiles of blk/2 rows
@@ -251,6 +259,10 @@ int li_sparse_attn(const li_problem *p, const int32_t *sel_idx, const int32_t *s
   ap.scale_log2 = scale * 1.4426950408889634f;
   ap.frame_idx = p->frame_idx; ap.sel_idx = sel_idx; ap.sel_cnt = sel_cnt;
   ap.o = (uint16_t *)o; ap.lse = lse_opt;
+  if (have_ws) {
+    ap.part_o = (float *)((char *)workspace + ws_bytes(p, dv));
+    ap.part_ml = (float2 *)((char *)ap.part_o + ws_split_o_bytes(p));
+  }
   int64_t n = 0;
   const int e = li::launch_attn(ap, dv.meta, p->d, blk, tm_q, tm_tk, tm_tv, tm_kf, tm_k8, tm_vf, tm_v8, (cudaStream_t)cuda_stream, &n);
   g_launches += n;

@@ -17,6 +17,8 @@
 // buffer once S has been read), [128,128+D) O.
 // On B200 this kernel runs into the 1 kW power cap (SM clock ~1.6 GHz under load); DESIGN.md section 6.3 lists the
 // measured alternatives (one CTA per SM with Q in tensor memory, two softmax groups, FMA-pipe exp2, ...).
+#include <cstdlib>
+
 #include "li_internal.h"
 #include "li_ptx.cuh"
 
@@ -62,7 +64,32 @@ enum {
   BAR_COUNT
 };
 
-template <int D, int BLK, bool K3D, bool TEXT>
+// n / dv for n, dv < 65536 by a multiply-high with mg = floor(2^32 / dv) + 1 (exact there: n * dv < 2^32)
+__device__ __forceinline__ int div_magic(int n, int dv, uint32_t mg) {
+  return (n | dv) < 65536 ? (int)__umulhi((uint32_t)n, mg) : n / dv;
+}
+
+// -inf into the key columns c of a half-tile with (c mod 32) >= V (compile-time positions: V..31 of every 32-row slice)
+template <int V, int HALF>
+__device__ __forceinline__ void mask_slice_tail(uint32_t (&s)[HALF]) {
+#pragma unroll
+  for (int c = 0; c < HALF; ++c)
+    if ((c & 31) >= V) s[c] = 0xff800000u;
+}
+
+// linear token of query row `row` of query block i, or -1 for a padding row ("masked stores")
+template <int BLK, bool K3D>
+__device__ __forceinline__ int64_t row_token(const AttnParams &p, int i, int row) {
+  if (K3D) {
+    const Tiling &tl = p.tl;
+    const int per = tl.Hb * tl.Wb, tg = i / per, hb = (i - tg * per) / tl.Wb, wb = i - tg * per - hb * tl.Wb;
+    const int f = tg * tl.bt + (row >> 5), within = row & 31, y = hb * tl.bh + within / tl.bw;
+    return (row < BLK && f < p.Lq / p.T_f && y < tl.gh) ? (int64_t)f * p.T_f + y * tl.gw + wb * tl.bw + within % tl.bw : -1;
+  }
+  return row < min(BLK, p.Lq - i * BLK) ? (int64_t)i * BLK + row : -1;
+}
+
+template <int D, int BLK, bool K3D, bool TEXT, bool SPLIT>
 __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &meta, const CUtensorMap &tm_q,
                                           const CUtensorMap &tm_k_full, const CUtensorMap &tm_k_8,
                                           const CUtensorMap &tm_v_full, const CUtensorMap &tm_v_8,
@@ -82,7 +109,17 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
   auto bar = [&](int i) { return bar0 + 8u * i; };
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int i = blockIdx.x, h = blockIdx.y, b = blockIdx.z;
+  // CTA -> (query block i, head h, call b) and, in the tail wave, which of n_split ranges of its half-tiles
+  // (SPLIT launches use a linear grid; the others the grid (Nqb, H, B) and none of this code)
+  int work = blockIdx.x, sq = 0, ns = 1;
+  if (SPLIT && work >= p.split_first) {
+    const int e = work - p.split_first;
+    work = p.split_first + e / p.n_split;
+    sq = e % p.n_split;
+    ns = p.n_split;
+  }
+  const int i = SPLIT ? work % p.Nqb : blockIdx.x, h = SPLIT ? (work / p.Nqb) % p.H : blockIdx.y,
+            b = SPLIT ? work / (p.Nqb * p.H) : blockIdx.z;
 
   // ---- per-tile integer bookkeeping (Eq. 11 context assembly) ----
   const int foff = meta.frame_off[b];
@@ -94,13 +131,19 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
   constexpr bool k3d = K3D;                            // 3-D blocks: BLK = bt*32, 32 = bh*bw rows per frame slice
   constexpr int SPH = HALF / 32;                       // 32-row slices per half-tile
   const int per = tl.Hb * tl.Wb;                       // blocks per temporal group (3-D)
+  // block index -> (temporal group, row block, column block)
+  auto split3 = [&](int blk, int &tg, int &hb, int &wb) {
+    tg = blk / per;
+    const int r = blk - tg * per;
+    hb = r / tl.Wb;
+    wb = r - hb * tl.Wb;
+  };
   const int M = tl.num_blocks(n_hist, p.T_f, BLK);
   const int Nc = tl.num_blocks(p.n_cur, p.T_f, BLK);
   const int n_qf = p.Lq / p.T_f;                       // query frames (3-D)
   const int Nt = TEXT ? (p.Lt + BLK - 1) / BLK : 0;    // text tiles (T of Eq. 11): dense, attended first, 1-D
   const int tail_text = p.Lt - (Nt - 1) * BLK;
   const int64_t row_id = ((int64_t)b * p.H + h) * p.Nqb + i;
-  const int valid_q = min(BLK, p.Lq - i * BLK);
   const int tail_cur = L_cur - (Nc - 1) * BLK, tail_hist = L_hist - (M - 1) * BLK;
 
   // ---- one-time setup (independent of the previous kernel: overlaps its tail under PDL) ----
@@ -149,9 +192,10 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
   };
   auto tile_blk = [&](int j) -> int { return j < Nt + Nc ? j - Nt : sel_at(j - Nt - Nc); };   // block index in its region
   auto tile_info = [&](int j) -> int {                 // 3-D: (frames of tile j that exist) | (valid rows per slice) << 8
-    const int blk = tile_blk(j);
-    const int nf = min(tl.bt, (j < Nt + Nc ? p.n_cur : n_hist) - (blk / per) * tl.bt);
-    return nf | (min(tl.bh, tl.gh - ((blk % per) / tl.Wb) * tl.bh) * tl.bw) << 8;
+    int tg, hb, wb;
+    split3(tile_blk(j), tg, hb, wb);
+    const int nf = min(tl.bt, (j < Nt + Nc ? p.n_cur : n_hist) - tg * tl.bt);
+    return nf | (min(tl.bh, tl.gh - hb * tl.bh) * tl.bw) << 8;
   };
   auto tile_info_cached = [&](int j) -> int { return j - Nt < kInfoCap ? (int)sInfo[j - Nt] : tile_info(j); };
   auto tile_frames = [&](int j) -> int { return tile_info_cached(j) & 0xff; };
@@ -177,17 +221,11 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
     if (j_tail_hist >= 0 && tail_hist <= HALF) --T;
   }
 
-  // linear token of query row `row` of this tile, or -1 for a padding row ("masked stores")
-  auto row_token = [&](int row) -> int64_t {
-    if (k3d) {
-      const int tg = i / per, hb = (i - tg * per) / tl.Wb, wb = i - tg * per - hb * tl.Wb;
-      const int f = tg * tl.bt + (row >> 5), within = row & 31, y = hb * tl.bh + within / tl.bw;
-      return (row < BLK && f < n_qf && y < tl.gh) ? (int64_t)f * p.T_f + y * tl.gw + wb * tl.bw + within % tl.bw : -1;
-    }
-    return row < valid_q ? (int64_t)i * BLK + row : -1;
-  };
+  // this CTA's range of half-tiles [t_lo, t_lo + Tn) (the whole list unless the query block is split)
+  const int t_lo = (SPLIT && ns > 1) ? (int)((int64_t)T * sq / ns) : 0;
+  const int Tn = (SPLIT && ns > 1) ? (int)((int64_t)T * (sq + 1) / ns) - t_lo : T;
 
-  if (T > 0) {
+  if (Tn > 0) {
     if (warp == 4) {
       // =============================== TMA producer ===============================
       // The warp stays converged (index arithmetic on warp-uniform values); an elected lane issues the TMA.
@@ -197,7 +235,8 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
         for (int c = 0; c < D / 64; ++c) {
           if (k3d) {
             // query block i = (tg, hb, wb): one 32-row box per frame; a frame past the chunk is out of bounds -> zeros
-            const int tg = i / per, hb = (i - tg * per) / tl.Wb, wb = i - tg * per - hb * tl.Wb;
+            int tg, hb, wb;
+            split3(i, tg, hb, wb);
             for (int tt = 0; tt < BLK / 32; ++tt)
               tma_load_5d(sQ + c * L::kQChunk + tt * 4096, &tm_q, bar(BAR_Q_FULL), c * 64, wb * tl.bw, hb * tl.bh,
                           min(tg * tl.bt + tt, n_qf), b * p.H + h);
@@ -207,6 +246,15 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
         }
       }
       __syncwarp();
+      // the producer splits a block index twice per half-tile: multiply-high instead of two integer divisions
+      const uint32_t mg_per = k3d ? 0xffffffffu / (uint32_t)max(per, 1) + 1u : 0u;   // (a divisor of 1 wraps to 0:
+      const uint32_t mg_wb = k3d ? 0xffffffffu / (uint32_t)max(tl.Wb, 1) + 1u : 0u;  //  handled in split3_fast)
+      auto split3_fast = [&](int blk, int &tg, int &hb, int &wb) {
+        tg = per > 1 ? div_magic(blk, per, mg_per) : blk;
+        const int r = blk - tg * per;
+        hb = tl.Wb > 1 ? div_magic(r, tl.Wb, mg_wb) : r;
+        wb = r - hb * tl.Wb;
+      };
       int n = 0;                                     // running load index: slot = n % 4
       // loads HALF rows [t0, t0+HALF) of a region (history or chunk) into ring slot n % 4
       auto load_half = [&](const CUtensorMap *tm_full, const CUtensorMap *tm_8, const CUtensorMap *tm_text, int j, int hh) {
@@ -232,7 +280,8 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
           // 5-D box (64 channels, bw, bh, head, page); grid rows >= grid_h are zero-filled by the hardware ("masked
           // loads"); a frame past the region's end is requested out of bounds -> zeros
           const int n_reg = is_cur ? p.n_cur : n_hist;
-          const int tg = blk / per, hb = (blk - tg * per) / tl.Wb, wb = blk - tg * per - hb * tl.Wb;
+          int tg, hb, wb;
+          split3_fast(blk, tg, hb, wb);
           int pg[SPH], y0[SPH];
 #pragma unroll
           for (int s = 0; s < SPH; ++s) {
@@ -295,11 +344,15 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
 
       // load order == consumption order of the MMA warp: K0 K1 | V0 K2 | V1 K3 | ...
       int kj = 0, kh = 0, vj = 0, vh = 0;
+      if (SPLIT) {                                   // split query block: skip to this CTA's range
+        for (int t = 0; t < t_lo; ++t) advance(kj, kh);
+        vj = kj; vh = kh;
+      }
       load_half(&tm_k_full, &tm_k_8, &tm_tk, kj, kh); advance(kj, kh);
-      if (T > 1) { load_half(&tm_k_full, &tm_k_8, &tm_tk, kj, kh); advance(kj, kh); }
-      for (int t = 0; t < T; ++t) {
+      if (Tn > 1) { load_half(&tm_k_full, &tm_k_8, &tm_tk, kj, kh); advance(kj, kh); }
+      for (int t = 0; t < Tn; ++t) {
         load_half(&tm_v_full, &tm_v_8, &tm_tv, vj, vh); advance(vj, vh);
-        if (t + 2 < T) { load_half(&tm_k_full, &tm_k_8, &tm_tk, kj, kh); advance(kj, kh); }
+        if (t + 2 < Tn) { load_half(&tm_k_full, &tm_k_8, &tm_tk, kj, kh); advance(kj, kh); }
       }
     } else if (warp == 5) {
       // =============================== MMA issuer ===============================
@@ -329,8 +382,8 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
       };
       mbar_wait(bar(BAR_Q_FULL), 0);
       issue_qk(0);
-      if (T > 1) issue_qk(1);
-      for (int t = 0; t < T; ++t) {
+      if (Tn > 1) issue_qk(1);
+      for (int t = 0; t < Tn; ++t) {
         // O += P(t) V(t)
         const int slot = c & (kStages - 1);
         const uint32_t sV = sRing + slot * L::kStage;
@@ -345,11 +398,11 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
                    (t > 0 || kk > 0) ? 1u : 0u);
           mma_commit(bar(BAR_EMPTY + slot));
           mma_commit(bar(BAR_PV_DONE));
-          if (t == T - 1) mma_commit(bar(BAR_O_FULL));
+          if (t == Tn - 1) mma_commit(bar(BAR_O_FULL));
         }
         __syncwarp();
         ++c;
-        if (t + 2 < T) issue_qk(t + 2);
+        if (t + 2 < Tn) issue_qk(t + 2);
       }
     } else {
       // =============================== softmax / lazy correction / epilogue ===============================
@@ -357,8 +410,14 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
       const int row = warp * 32 + lane;                // query row inside the tile == TMEM lane
       float m_used = 0.f, l = 0.f;
       int j = 0, hh = 0;
+      if (SPLIT) {                                     // split query block: skip to this CTA's range
+        for (int t = 0; t < t_lo; ++t) {
+          if (hh == 0 && halves(j) > 1) hh = 1;
+          else { ++j; hh = 0; }
+        }
+      }
 
-      for (int t = 0; t < T; ++t) {
+      for (int t = 0; t < Tn; ++t) {
         // valid key columns of this half-tile, as a prefix length per 32-column slice (vs[s] rows of slice s are real,
         // the rest is padding): 1-D blocks have one valid prefix; a 3-D slice is one frame's bh x bw patch, whose
         // grid rows beyond grid_h (and whose frame, beyond the region) are padding
@@ -386,8 +445,18 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
         for (int c = 0; c < HALF / 32; ++c) tmem_ld32(s_addr + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&s[c * 32]));
         tc_wait_ld();
         if (!full) {                                   // padded key columns -> -inf (warp-uniform branch)
+          bool same = k3d;                               // 3-D border tile: every slice has the same valid prefix,
 #pragma unroll
-          for (int c = 0; c < HALF; ++c) if ((c & 31) >= vs[c >> 5]) s[c] = 0xff800000u;
+          for (int s_ = 1; s_ < SPH; ++s_) same = same && vs[s_] == vs[0];   // a multiple of bw rows
+          if (same && (vs[0] & 7) == 0 && vs[0] > 0) {
+            // compile-time column positions: a few moves, no compares
+            if (vs[0] == 24) mask_slice_tail<24, HALF>(s);
+            else if (vs[0] == 16) mask_slice_tail<16, HALF>(s);
+            else mask_slice_tail<8, HALF>(s);
+          } else {
+#pragma unroll
+            for (int c = 0; c < HALF; ++c) if ((c & 31) >= vs[c >> 5]) s[c] = 0xff800000u;
+          }
         }
         float mx0 = __uint_as_float(s[0]), mx1 = __uint_as_float(s[1]), mx2 = __uint_as_float(s[2]), mx3 = __uint_as_float(s[3]);
 #pragma unroll
@@ -454,41 +523,62 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
         if (lane == 0) mbar_arrive(bar(BAR_P_FULL + (t & 1)));
       }
 
-      // epilogue: O / l -> bf16, stored in linear token order (no untile pass)
       mbar_wait(bar(BAR_O_FULL), 0);
       tc_fence_after();
-      const float inv_l = 1.0f / l;
-      const int64_t u = row_token(row);
-      const bool live = u >= 0;
-      uint16_t *orow = p.o + (((int64_t)b * p.H + h) * p.Lq + u) * D;
+      if (SPLIT && ns > 1) {
+        // split query block: unnormalised fp32 partial O and (reference maximum, row sum) for li_attn_combine_kernel
+        const int64_t prow = (int64_t)(blockIdx.x - p.split_first) * 128 + row;
+        float *po = p.part_o + prow * D;
 #pragma unroll
-      for (int c = 0; c < D / 32; ++c) {
-        uint32_t o[32];
-        tmem_ld32(tmem + lane_base + kOCol + c * 32, o);
-        tc_wait_ld();
-        if (live) {
+        for (int c = 0; c < D / 32; ++c) {
+          uint32_t o[32];
+          tmem_ld32(tmem + lane_base + kOCol + c * 32, o);
+          tc_wait_ld();
 #pragma unroll
-          for (int e = 0; e < 32; e += 8) {
-            uint4 v;
-            v.x = pack_bf16x2(__uint_as_float(o[e + 0]) * inv_l, __uint_as_float(o[e + 1]) * inv_l);
-            v.y = pack_bf16x2(__uint_as_float(o[e + 2]) * inv_l, __uint_as_float(o[e + 3]) * inv_l);
-            v.z = pack_bf16x2(__uint_as_float(o[e + 4]) * inv_l, __uint_as_float(o[e + 5]) * inv_l);
-            v.w = pack_bf16x2(__uint_as_float(o[e + 6]) * inv_l, __uint_as_float(o[e + 7]) * inv_l);
-            *reinterpret_cast<uint4 *>(orow + c * 32 + e) = v;
+          for (int e = 0; e < 32; e += 4)
+            *reinterpret_cast<uint4 *>(po + c * 32 + e) = make_uint4(o[e], o[e + 1], o[e + 2], o[e + 3]);
+        }
+        p.part_ml[prow] = make_float2(m_used, l);
+      } else {
+        // epilogue: O / l -> bf16, stored in linear token order (no untile pass)
+        const float inv_l = 1.0f / l;
+        const int64_t u = row_token<BLK, K3D>(p, i, row);
+        const bool live = u >= 0;
+        uint16_t *orow = p.o + (((int64_t)b * p.H + h) * p.Lq + u) * D;
+#pragma unroll
+        for (int c = 0; c < D / 32; ++c) {
+          uint32_t o[32];
+          tmem_ld32(tmem + lane_base + kOCol + c * 32, o);
+          tc_wait_ld();
+          if (live) {
+#pragma unroll
+            for (int e = 0; e < 32; e += 8) {
+              uint4 v;
+              v.x = pack_bf16x2(__uint_as_float(o[e + 0]) * inv_l, __uint_as_float(o[e + 1]) * inv_l);
+              v.y = pack_bf16x2(__uint_as_float(o[e + 2]) * inv_l, __uint_as_float(o[e + 3]) * inv_l);
+              v.z = pack_bf16x2(__uint_as_float(o[e + 4]) * inv_l, __uint_as_float(o[e + 5]) * inv_l);
+              v.w = pack_bf16x2(__uint_as_float(o[e + 6]) * inv_l, __uint_as_float(o[e + 7]) * inv_l);
+              *reinterpret_cast<uint4 *>(orow + c * 32 + e) = v;
+            }
           }
         }
+        if (live && p.lse != nullptr)
+          p.lse[((int64_t)b * p.H + h) * p.Lq + u] = (m_used + log2f(l)) * 0.6931471805599453f;
       }
-      if (live && p.lse != nullptr)
-        p.lse[((int64_t)b * p.H + h) * p.Lq + u] = (m_used + log2f(l)) * 0.6931471805599453f;
     }
   } else {
-    // empty context: o = 0, lse = -inf
+    // no half-tile for this CTA (empty context, or a split range without tiles)
     if (warp < 4) {
-      const int64_t u = row_token(warp * 32 + lane);
-      if (u >= 0) {
-        uint16_t *orow = p.o + (((int64_t)b * p.H + h) * p.Lq + u) * D;
-        for (int c = 0; c < D; c += 8) *reinterpret_cast<uint4 *>(orow + c) = make_uint4(0, 0, 0, 0);
-        if (p.lse != nullptr) p.lse[((int64_t)b * p.H + h) * p.Lq + u] = __int_as_float(0xff800000);
+      const int row = warp * 32 + lane;
+      if (SPLIT && ns > 1) {
+        p.part_ml[(int64_t)(blockIdx.x - p.split_first) * 128 + row] = make_float2(0.f, 0.f);   // row sum 0: ignored
+      } else {
+        const int64_t u = row_token<BLK, K3D>(p, i, row);   // o = 0, lse = -inf
+        if (u >= 0) {
+          uint16_t *orow = p.o + (((int64_t)b * p.H + h) * p.Lq + u) * D;
+          for (int c = 0; c < D; c += 8) *reinterpret_cast<uint4 *>(orow + c) = make_uint4(0, 0, 0, 0);
+          if (p.lse != nullptr) p.lse[((int64_t)b * p.H + h) * p.Lq + u] = __int_as_float(0xff800000);
+        }
       }
     }
   }
@@ -500,59 +590,131 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
 
 // Two entry points: the text maps are kernel parameters only of the variant that attends a text prefix (adding two
 // unused 128-byte tensor maps to the parameter block of the plain kernel measurably slowed it down).
-template <int D, int BLK, bool K3D>
+template <int D, int BLK, bool K3D, bool SPLIT>
 __global__ void __launch_bounds__(192, 2)
 li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_constant__ CUtensorMap tm_q,
                       const __grid_constant__ CUtensorMap tm_k_full, const __grid_constant__ CUtensorMap tm_k_8,
                       const __grid_constant__ CUtensorMap tm_v_full, const __grid_constant__ CUtensorMap tm_v_8) {
-  attn_body<D, BLK, K3D, false>(p, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, tm_q, tm_q);
+  attn_body<D, BLK, K3D, false, SPLIT>(p, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, tm_q, tm_q);
 }
 
-template <int D, int BLK, bool K3D>
+template <int D, int BLK, bool K3D, bool SPLIT>
 __global__ void __launch_bounds__(192, 2)
 li_sparse_attn_text_kernel(const AttnParams p, const BatchMeta meta, const __grid_constant__ CUtensorMap tm_q,
                            const __grid_constant__ CUtensorMap tm_k_full, const __grid_constant__ CUtensorMap tm_k_8,
                            const __grid_constant__ CUtensorMap tm_v_full, const __grid_constant__ CUtensorMap tm_v_8,
                            const __grid_constant__ CUtensorMap tm_tk, const __grid_constant__ CUtensorMap tm_tv) {
-  attn_body<D, BLK, K3D, true>(p, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, tm_tk, tm_tv);
+  attn_body<D, BLK, K3D, true, SPLIT>(p, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, tm_tk, tm_tv);
 }
 
-template <int D, int BLK, bool K3D, bool TEXT>
+// Merges the n_split partial results of every split query block (tail-wave split): with reference maxima
+// m_q and row sums l_q, O = sum_q 2^(m_q - M) O_q / sum_q 2^(m_q - M) l_q, M = max_q m_q over the parts that saw a key.
+// grid (split query blocks, 16), 8 warps: one warp per query row, lane = D/32 consecutive channels.
+template <int D, int BLK, bool K3D>
+__global__ void __launch_bounds__(256) li_attn_combine_kernel(const AttnParams p) {
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int work = p.split_first + blockIdx.x, row = blockIdx.y * 8 + warp;
+  const int i = work % p.Nqb, h = (work / p.Nqb) % p.H, b = work / (p.Nqb * p.H);
+  const int64_t u = row_token<BLK, K3D>(p, i, row);
+  if (u < 0) return;
+  constexpr int V = D / 32;
+  const int64_t prow0 = (int64_t)blockIdx.x * p.n_split * 128 + row;
+  float M = __int_as_float(0xff800000);
+  for (int q = 0; q < p.n_split; ++q) {
+    const float2 ml = p.part_ml[prow0 + (int64_t)q * 128];
+    if (ml.y > 0.f) M = fmaxf(M, ml.x);
+  }
+  float L = 0.f, acc[V];
+#pragma unroll
+  for (int c = 0; c < V; ++c) acc[c] = 0.f;
+  for (int q = 0; q < p.n_split; ++q) {
+    const float2 ml = p.part_ml[prow0 + (int64_t)q * 128];
+    if (ml.y > 0.f) {
+      const float w = exp2f(ml.x - M);
+      L += w * ml.y;
+      const float *po = p.part_o + (prow0 + (int64_t)q * 128) * D + lane * V;
+#pragma unroll
+      for (int c = 0; c < V; ++c) acc[c] += w * po[c];
+    }
+  }
+  const float inv = L > 0.f ? 1.0f / L : 0.f;
+  uint16_t *orow = p.o + (((int64_t)b * p.H + h) * p.Lq + u) * D + lane * V;
+#pragma unroll
+  for (int c = 0; c < V; c += 2) *reinterpret_cast<uint32_t *>(orow + c) = pack_bf16x2(acc[c] * inv, acc[c + 1] * inv);
+  if (lane == 0 && p.lse != nullptr)
+    p.lse[((int64_t)b * p.H + h) * p.Lq + u] = L > 0.f ? (M + log2f(L)) * 0.6931471805599453f : __int_as_float(0xff800000);
+}
+
+template <int D, int BLK, bool K3D, bool TEXT, bool SPLIT>
 static int launch_one(const AttnParams &ap, const BatchMeta &meta, const CUtensorMap &tm_q, const CUtensorMap &tm_tk,
                       const CUtensorMap &tm_tv, const CUtensorMap &tm_k_full,
                       const CUtensorMap &tm_k_8, const CUtensorMap &tm_v_full, const CUtensorMap &tm_v_8,
                       cudaStream_t st) {
   constexpr int smem = AttnSmem<D, BLK>::kTotal;
   cudaError_t e;
-  if constexpr (TEXT) e = cudaFuncSetAttribute(li_sparse_attn_text_kernel<D, BLK, K3D>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-  else e = cudaFuncSetAttribute(li_sparse_attn_kernel<D, BLK, K3D>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  if constexpr (TEXT) e = cudaFuncSetAttribute(li_sparse_attn_text_kernel<D, BLK, K3D, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  else e = cudaFuncSetAttribute(li_sparse_attn_kernel<D, BLK, K3D, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   if (e != cudaSuccess) return (int)e;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(ap.Nqb, ap.H, ap.B);
+  const int n_work = ap.Nqb * ap.H * ap.B;
+  cfg.gridDim = SPLIT ? dim3(ap.split_first + (n_work - ap.split_first) * ap.n_split) : dim3(ap.Nqb, ap.H, ap.B);
   cfg.blockDim = dim3(192);
   cfg.dynamicSmemBytes = smem;
   cfg.stream = st;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
   if constexpr (TEXT)
-    e = cudaLaunchKernelEx(&cfg, li_sparse_attn_text_kernel<D, BLK, K3D>, ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, tm_tk, tm_tv);
+    e = cudaLaunchKernelEx(&cfg, li_sparse_attn_text_kernel<D, BLK, K3D, SPLIT>, ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, tm_tk, tm_tv);
   else
-    e = cudaLaunchKernelEx(&cfg, li_sparse_attn_kernel<D, BLK, K3D>, ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8);
+    e = cudaLaunchKernelEx(&cfg, li_sparse_attn_kernel<D, BLK, K3D, SPLIT>, ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8);
   if (e != cudaSuccess) return (int)e;
+  if (SPLIT) {
+    cfg.gridDim = dim3(n_work - ap.split_first, 16);
+    cfg.blockDim = dim3(256);
+    cfg.dynamicSmemBytes = 0;
+    e = cudaLaunchKernelEx(&cfg, li_attn_combine_kernel<D, BLK, K3D>, ap);
+    if (e != cudaSuccess) return (int)e;
+  }
   return (int)cudaGetLastError();
 }
 
-int launch_attn(const AttnParams &ap, const BatchMeta &meta, int d, int blk, const CUtensorMap &tm_q,
+int launch_attn(const AttnParams &ap_in, const BatchMeta &meta, int d, int blk, const CUtensorMap &tm_q,
                 const CUtensorMap &tm_tk, const CUtensorMap &tm_tv, const CUtensorMap &tm_k_full, const CUtensorMap &tm_k_8, const CUtensorMap &tm_v_full,
                 const CUtensorMap &tm_v_8, cudaStream_t st, int64_t *n_launches) {
   int e;
+  AttnParams ap = ap_in;
   const bool k3 = ap.tl.bt > 0;
-#define LI_LAUNCH2(DD, BB, K3)                                                                               \
-  (ap.Lt > 0 ? launch_one<DD, BB, K3, true>(ap, meta, tm_q, tm_tk, tm_tv, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st)  \
-             : launch_one<DD, BB, K3, false>(ap, meta, tm_q, tm_tk, tm_tv, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st))
+  // Tail-wave split.  The GPU holds `slots` = 2 CTAs per SM at a time; when the last wave would fill at
+  // most half of them, its `rem` query blocks are each shared by s CTAs (s * rem <= slots), so the tail takes ~1/s of
+  // a wave.  Needs the partial-result buffers (caller passed a full-size workspace); LI_SPLIT_KV=0 turns it off.
+  const int n_work = ap.Nqb * ap.H * ap.B;
+  ap.split_first = n_work;
+  ap.n_split = 1;
+  int dev = 0, n_sm = 0;
+  const char *env = std::getenv("LI_SPLIT_KV");
+  if (ap.part_o != nullptr && !(env != nullptr && env[0] == '0') && cudaGetDevice(&dev) == cudaSuccess &&
+      cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n_sm > 0) {
+    const int wave = 2 * n_sm, slots = wave < kMaxSplitSlots ? wave : kMaxSplitSlots;
+    const int rem = n_work % wave;
+    if (rem > 0 && 2 * rem <= slots) {
+      const int t_est = 2 * ((ap.Lt + blk - 1) / blk + ap.Nc + ap.kmax);   // half-tiles per query block, upper bound
+      int s = slots / rem;
+      if (s > 8) s = 8;
+      if (s > t_est / 16) s = t_est / 16;               // at least ~16 half-tiles per CTA
+      if (s >= 2) {
+        ap.n_split = s;
+        ap.split_first = n_work - rem;
+      }
+    }
+  }
+#define LI_LAUNCH3(DD, BB, K3, TX)                                                                                    \
+  (ap.n_split > 1 ? launch_one<DD, BB, K3, TX, true>(ap, meta, tm_q, tm_tk, tm_tv, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st) \
+                  : launch_one<DD, BB, K3, TX, false>(ap, meta, tm_q, tm_tk, tm_tv, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st))
+#define LI_LAUNCH2(DD, BB, K3) (ap.Lt > 0 ? LI_LAUNCH3(DD, BB, K3, true) : LI_LAUNCH3(DD, BB, K3, false))
 #define LI_LAUNCH(DD, BB) (k3 ? LI_LAUNCH2(DD, BB, true) : LI_LAUNCH2(DD, BB, false))
   if (d == 128 && blk == 128) e = LI_LAUNCH(128, 128);
   else if (d == 128 && blk == 64) e = LI_LAUNCH(128, 64);
@@ -560,7 +722,8 @@ int launch_attn(const AttnParams &ap, const BatchMeta &meta, int d, int blk, con
   else e = LI_LAUNCH(64, 64);
 #undef LI_LAUNCH
 #undef LI_LAUNCH2
-  if (e == 0 && n_launches) *n_launches += 1;
+#undef LI_LAUNCH3
+  if (e == 0 && n_launches) *n_launches += ap.n_split > 1 ? 2 : 1;
   return e;
 }
 

@@ -53,7 +53,15 @@ struct AttnParams {
   const int32_t *sel_cnt;
   uint16_t *o;
   float *lse;
+  // tail-wave split: CTAs [0, split_first) own a whole query block each; from split_first on, n_split
+  // consecutive CTAs share one query block, each taking a contiguous range of its half-tiles and writing unnormalised
+  // partial results, which li_attn_combine_kernel merges.  n_split == 1: no split (split_first == number of blocks).
+  int32_t split_first, n_split;
+  float *part_o;    // [slot][128 rows][d] fp32, slot = CTA - split_first
+  float2 *part_ml;  // [slot][128 rows] (reference maximum in log2 units, row sum)
 };
+
+constexpr int kMaxSplitSlots = 320;   // upper bound of split CTAs (<= 2 CTAs per SM), sizes the workspace
 
 // launches (defined in the .cu files); return cudaError_t as int
 int launch_select(const SelectParams &sp, const BatchMeta &meta, cudaStream_t st, int64_t *n_launches);

@@ -72,7 +72,8 @@ def test_workspace_bytes_and_validation(L):
     ws = L.li_workspace_bytes(ctypes.byref(p), 8)
     # qbar [1,2,4,64] fp32 + kbar [1,2,64,32] fp32 (transposed, M padded to 32) + score keys [1,2,4,12] u32,
     # each rounded up to 256 B
-    assert ws == 2 * 4 * 64 * 4 + 2 * 64 * 32 * 4 + 512
+    # + the attention kernel's split buffers: 320 slots x 128 rows x (d fp32 + one float2)
+    assert ws == 2 * 4 * 64 * 4 + 2 * 64 * 32 * 4 + 512 + 320 * 128 * (64 * 4 + 8)
     tk = np.asarray([8], dtype=np.int32)
 
     def select(prob, kmax=8, ws_ptr=0x50000, ws_bytes=ws, sel=0x60000, cnt=0x70000):
@@ -114,7 +115,8 @@ def test_3d_tiling_validation(L):
     p, keep = prob3d()
     # history 4 frames -> 1 temporal group x 4 x 13 = 52 blocks; Nqb = 52 (chunk of 2 frames = one partial group)
     ws = L.li_workspace_bytes(ctypes.byref(p), 8)
-    assert ws == 24 * 52 * 128 * 4 + 24 * 128 * 64 * 4 + 24 * 52 * 52 * 4 + (256 - (24 * 52 * 52 * 4) % 256) % 256
+    assert ws == (24 * 52 * 128 * 4 + 24 * 128 * 64 * 4 + 24 * 52 * 52 * 4 + (256 - (24 * 52 * 52 * 4) % 256) % 256
+                  + 320 * 128 * (128 * 4 + 8))
     for bad, code in ((dict(bw=8), li.LI_ERR_UNSUPPORTED),            # 4*8*8 != 128
                       (dict(bh=4, bw=8), li.LI_ERR_UNSUPPORTED),       # 52 % 8 != 0
                       (dict(grid_w=50), li.LI_ERR_INVALID_ARG),        # grid_h*grid_w != frame_tokens
