@@ -29,8 +29,8 @@ force; exact ties -> lowest index; k=M; nested selections.
 The 3-D block tiling of PAPER.md:129/:321 (functions *_3d at the end) is pinned by tests/test_oracle_3d_pins.py:
 explicit coordinate brute force, reduction to the 1-D tiling when blocks are row segments, partition and padding
 properties.  The text set T of Eq. 11 (text_k / text_v arguments) is pinned in the same files (brute force, dense SDPA over
-[text | context], text-only attention).  Nothing in this file is "parity unpinned".  (The policy scalars of Eq. 1-8
-are not implemented here at all: out of the hot-path scope.)
+[text | context], text-only attention).  Nothing in this file is "parity unpinned".  (The context policy of Eq. 1-4 has
+its own oracle, li_policy_oracle.py; Eq. 5-8, the denoising cache, are out of the hot-path scope.)
 """
 from __future__ import annotations
 
