@@ -36,7 +36,7 @@
 extern "C" {
 #endif
 
-#define LI_VERSION 100          /* major*100 + minor */
+#define LI_VERSION 101          /* major*100 + minor */
 #define LI_MAX_CALLS 64         /* max B per call of the library (batch of independent attention calls) */
 
 enum {
@@ -121,7 +121,52 @@ int li_sparse_attn(const li_problem *p, const int32_t *sel_idx, const int32_t *s
  * followed by the partial-result buffers of li_sparse_attn's split (a fixed ~21 MB at d = 128). */
 size_t li_workspace_bytes(const li_problem *p, int32_t kmax);
 
-/* Number of kernel launches the two calls above issued since the last li_reset_launch_count()
+/* Adaptive context management and the frame list it produces -- what li_problem.frame_idx is built from,
+ * once per chunk.  All pointers are DEVICE pointers; nothing is read back by the call.
+ *   Eq. 1  D_t    = mean over all n_latent dimensions of (z_prev1 - z_prev2)^2         (fp32 products, fp64 sums)
+ *   Eq. 2  Dbar_t = alpha D_t + (1 - alpha) Dbar_{t-1}; ema_state = {Dbar, valid}: valid == 0 -> Dbar_t = D_t; updated
+ *          in place (fp32)
+ *   Eq. 3  L_t    = clip([L_max * kappa / (Dbar_t + kappa)], 1, L_max) in fp32, evaluated as (L_max*kappa)/(Dbar_t+kappa);
+ *          the bracket (garbled in the paper) is floor, or round-half-to-even when round_nearest != 0
+ *   Eq. 4  keep_memory = !(max_j s_pose[j] < tau_pose); no candidate (n_cand == 0) -> 0
+ *   frame_idx_out = [mem_pages[0..n_mem) if keep_memory] + [the min(L_t, n_win) LAST entries of win_pages (oldest ->
+ *          newest)] + [cur_pages[0..n_cur)]. */
+typedef struct li_policy {
+  const void *z_prev1;          /* latents of the two most recent stable units, 16-byte aligned */
+  const void *z_prev2;
+  int64_t n_latent;             /* elements of each */
+  int32_t latent_bf16;          /* 0: fp32, 1: bf16 */
+  float alpha;                  /* in (0, 1] */
+  float kappa;                  /* > 0 */
+  int32_t L_max;                /* L_m of Eq. 3, >= 1 */
+  int32_t round_nearest;        /* Eq. 3 bracket: 0 floor, 1 nearest */
+  float *ema_state;             /* float[2] */
+  const float *s_pose;          /* fp32 [n_cand] (may be NULL when n_cand == 0) */
+  int32_t n_cand;
+  float tau_pose;
+  const int32_t *mem_pages;     /* int32 [n_mem] */
+  int32_t n_mem;
+  const int32_t *win_pages;     /* int32 [n_win] */
+  int32_t n_win;
+  const int32_t *cur_pages;     /* int32 [n_cur] */
+  int32_t n_cur;
+} li_policy;
+
+typedef struct li_policy_result {   /* written to DEVICE memory by li_context_policy */
+  float D_t, D_bar;
+  int32_t L_t, keep_memory;
+  int32_t n_hist_frames;        /* (kept memory) + (window frames used) */
+  int32_t n_frames;             /* entries written to frame_idx_out = n_hist_frames + n_cur */
+} li_policy_result;
+
+/* frame_idx_capacity must be >= n_mem + min(L_max, n_win) + n_cur (entries past n_frames are left untouched);
+ * workspace >= li_policy_workspace_bytes() bytes, 256-byte aligned.  Two kernel launches, no host synchronisation: the
+ * caller reads result_dev back (24 bytes) when it needs the frame count on the host (li_problem.frame_off_host). */
+int li_context_policy(const li_policy *pp, int32_t *frame_idx_out, int32_t frame_idx_capacity,
+                      li_policy_result *result_dev, void *workspace, size_t workspace_bytes, void *cuda_stream);
+size_t li_policy_workspace_bytes(void);
+
+/* Number of kernel launches the calls above issued since the last li_reset_launch_count()
  * (bench.py's gpu_launches). */
 int64_t li_launch_count(void);
 void li_reset_launch_count(void);

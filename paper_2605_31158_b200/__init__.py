@@ -19,8 +19,8 @@ LIB_PATH = os.path.join(_HERE, "libli.so")
 LI_OK, LI_ERR_INVALID_ARG, LI_ERR_UNSUPPORTED, LI_ERR_WORKSPACE, LI_ERR_CUDA = 0, -1, -2, -3, -4
 LI_MAX_CALLS = 64
 
-EXPORTS = ("li_block_select", "li_block_select_reuse_kbar", "li_sparse_attn", "li_workspace_bytes", "li_launch_count",
-           "li_reset_launch_count", "li_strerror", "li_version")
+EXPORTS = ("li_block_select", "li_block_select_reuse_kbar", "li_sparse_attn", "li_workspace_bytes", "li_context_policy",
+           "li_policy_workspace_bytes", "li_launch_count", "li_reset_launch_count", "li_strerror", "li_version")
 
 
 class LiError(RuntimeError):
@@ -47,6 +47,25 @@ class li_problem(ctypes.Structure):
     ]
 
 
+class li_policy(ctypes.Structure):
+    """Mirror of `struct li_policy` in include/li.h."""
+    _fields_ = [
+        ("z_prev1", ctypes.c_void_p), ("z_prev2", ctypes.c_void_p), ("n_latent", ctypes.c_int64),
+        ("latent_bf16", ctypes.c_int32), ("alpha", ctypes.c_float), ("kappa", ctypes.c_float),
+        ("L_max", ctypes.c_int32), ("round_nearest", ctypes.c_int32), ("ema_state", ctypes.c_void_p),
+        ("s_pose", ctypes.c_void_p), ("n_cand", ctypes.c_int32), ("tau_pose", ctypes.c_float),
+        ("mem_pages", ctypes.c_void_p), ("n_mem", ctypes.c_int32),
+        ("win_pages", ctypes.c_void_p), ("n_win", ctypes.c_int32),
+        ("cur_pages", ctypes.c_void_p), ("n_cur", ctypes.c_int32),
+    ]
+
+
+class li_policy_result(ctypes.Structure):
+    """Mirror of `struct li_policy_result` in include/li.h (24 bytes, written to device memory)."""
+    _fields_ = [("D_t", ctypes.c_float), ("D_bar", ctypes.c_float), ("L_t", ctypes.c_int32),
+                ("keep_memory", ctypes.c_int32), ("n_hist_frames", ctypes.c_int32), ("n_frames", ctypes.c_int32)]
+
+
 _lib = None
 
 
@@ -70,6 +89,11 @@ def lib() -> ctypes.CDLL:
         L.li_sparse_attn.restype = ctypes.c_int
         L.li_sparse_attn.argtypes = [P, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p,
                                      ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p]
+        L.li_policy_workspace_bytes.restype = ctypes.c_size_t
+        L.li_policy_workspace_bytes.argtypes = []
+        L.li_context_policy.restype = ctypes.c_int
+        L.li_context_policy.argtypes = [ctypes.POINTER(li_policy), ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p,
+                                        ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p]
         L.li_launch_count.restype = ctypes.c_int64
         L.li_reset_launch_count.restype = None
         L.li_strerror.restype = ctypes.c_char_p
@@ -218,3 +242,46 @@ def forward(ctx: Context, top_k: Sequence[int], buf: Buffers,
     li_block_select(ctx, top_k, buf.kmax, buf.sel_idx, buf.sel_cnt, buf.workspace, buf.scores, stream)
     li_sparse_attn(ctx, buf.sel_idx, buf.sel_cnt, buf.kmax, buf.o, buf.lse, buf.workspace, stream)
     return buf.o, buf.lse
+
+
+def li_context_policy(z_prev1: torch.Tensor, z_prev2: torch.Tensor, ema_state: torch.Tensor, alpha: float, kappa: float,
+                      L_max: int, s_pose: Optional[torch.Tensor], tau_pose: float, mem_pages: Optional[torch.Tensor],
+                      win_pages: Optional[torch.Tensor], cur_pages: torch.Tensor, frame_idx_out: torch.Tensor,
+                      result: torch.Tensor, workspace: torch.Tensor, round_nearest: bool = False,
+                      stream: Optional[torch.cuda.Stream] = None) -> None:
+    """li_context_policy (include/li.h; Eq. 1-4).  All tensors live on the GPU: latents fp32 or bf16 (contiguous),
+    ema_state fp32 [2], s_pose fp32 [n_cand], page lists int32, frame_idx_out int32 [capacity], result uint8 [24]
+    (read it with `policy_result`), workspace uint8 [>= li_policy_workspace_bytes]."""
+    if z_prev1.shape != z_prev2.shape or z_prev1.dtype != z_prev2.dtype or z_prev1.dtype not in (torch.float32, torch.bfloat16):
+        raise ValueError("latents must be two fp32 or bf16 tensors of the same shape")
+    tensors = [z_prev1, z_prev2, ema_state, cur_pages, frame_idx_out, result, workspace] + \
+              [t for t in (s_pose, mem_pages, win_pages) if t is not None]
+    if not all(t.is_cuda and t.is_contiguous() for t in tensors):
+        raise ValueError("li_context_policy takes contiguous CUDA tensors")
+    for t, dt, name in ((ema_state, torch.float32, "ema_state"), (s_pose, torch.float32, "s_pose"),
+                        (mem_pages, torch.int32, "mem_pages"), (win_pages, torch.int32, "win_pages"),
+                        (cur_pages, torch.int32, "cur_pages"), (frame_idx_out, torch.int32, "frame_idx_out")):
+        if t is not None and t.dtype != dt:
+            raise ValueError(f"{name} must be {dt}")
+    if ema_state.numel() < 2 or result.numel() * result.element_size() < ctypes.sizeof(li_policy_result):
+        raise ValueError("ema_state needs 2 floats, result 24 bytes")
+    pp = li_policy()
+    pp.z_prev1, pp.z_prev2, pp.n_latent = z_prev1.data_ptr(), z_prev2.data_ptr(), z_prev1.numel()
+    pp.latent_bf16 = 1 if z_prev1.dtype == torch.bfloat16 else 0
+    pp.alpha, pp.kappa, pp.L_max, pp.round_nearest = float(alpha), float(kappa), int(L_max), 1 if round_nearest else 0
+    pp.ema_state = ema_state.data_ptr()
+    pp.s_pose, pp.n_cand, pp.tau_pose = (s_pose.data_ptr() if s_pose is not None else None,
+                                         s_pose.numel() if s_pose is not None else 0, float(tau_pose))
+    pp.mem_pages, pp.n_mem = (mem_pages.data_ptr(), mem_pages.numel()) if mem_pages is not None else (None, 0)
+    pp.win_pages, pp.n_win = (win_pages.data_ptr(), win_pages.numel()) if win_pages is not None else (None, 0)
+    pp.cur_pages, pp.n_cur = cur_pages.data_ptr(), cur_pages.numel()
+    rc = lib().li_context_policy(ctypes.byref(pp), frame_idx_out.data_ptr(), frame_idx_out.numel(), result.data_ptr(),
+                                 workspace.data_ptr(), workspace.numel() * workspace.element_size(), _stream_ptr(stream))
+    if rc != LI_OK:
+        raise LiError(rc, "li_context_policy")
+
+
+def policy_result(result: torch.Tensor) -> li_policy_result:
+    """Copies the 24-byte li_policy_result record to the host (synchronises on the copy)."""
+    raw = result.cpu().numpy().tobytes()[:ctypes.sizeof(li_policy_result)]
+    return li_policy_result.from_buffer_copy(raw)

@@ -271,6 +271,29 @@ int li_sparse_attn(const li_problem *p, const int32_t *sel_idx, const int32_t *s
   return e == 0 ? LI_OK : LI_ERR_CUDA;
 }
 
+size_t li_policy_workspace_bytes(void) { return li::kPolicyWorkspaceBytes; }
+
+int li_context_policy(const li_policy *pp, int32_t *frame_idx_out, int32_t frame_idx_capacity, li_policy_result *result_dev,
+                      void *workspace, size_t workspace_bytes, void *cuda_stream) {
+  if (pp == nullptr || frame_idx_out == nullptr || result_dev == nullptr) return LI_ERR_INVALID_ARG;
+  if (pp->z_prev1 == nullptr || pp->z_prev2 == nullptr || pp->n_latent <= 0) return LI_ERR_INVALID_ARG;
+  if (((uintptr_t)pp->z_prev1 & 15u) || ((uintptr_t)pp->z_prev2 & 15u)) return LI_ERR_INVALID_ARG;
+  if (pp->latent_bf16 != 0 && pp->latent_bf16 != 1) return LI_ERR_INVALID_ARG;
+  if (!(pp->alpha > 0.f && pp->alpha <= 1.f) || !(pp->kappa > 0.f) || pp->L_max < 1) return LI_ERR_INVALID_ARG;
+  if (pp->ema_state == nullptr) return LI_ERR_INVALID_ARG;
+  if (pp->n_cand < 0 || pp->n_mem < 0 || pp->n_win < 0 || pp->n_cur < 0) return LI_ERR_INVALID_ARG;
+  if ((pp->n_cand > 0 && pp->s_pose == nullptr) || (pp->n_mem > 0 && pp->mem_pages == nullptr) ||
+      (pp->n_win > 0 && pp->win_pages == nullptr) || (pp->n_cur > 0 && pp->cur_pages == nullptr))
+    return LI_ERR_INVALID_ARG;
+  const int64_t need = (int64_t)pp->n_mem + (pp->L_max < pp->n_win ? pp->L_max : pp->n_win) + pp->n_cur;
+  if (frame_idx_capacity < need) return LI_ERR_INVALID_ARG;
+  if (workspace == nullptr || workspace_bytes < li::kPolicyWorkspaceBytes || ((uintptr_t)workspace & 255u)) return LI_ERR_WORKSPACE;
+  int64_t n = 0;
+  const int e = li::launch_policy(*pp, frame_idx_out, result_dev, (double *)workspace, (cudaStream_t)cuda_stream, &n);
+  g_launches += n;
+  return e == 0 ? LI_OK : LI_ERR_CUDA;
+}
+
 int64_t li_launch_count(void) { return g_launches.load(); }
 void li_reset_launch_count(void) { g_launches.store(0); }
 

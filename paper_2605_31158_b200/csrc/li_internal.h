@@ -69,4 +69,8 @@ int launch_attn(const AttnParams &ap, const BatchMeta &meta, int d, int blk, con
                 const CUtensorMap &tm_tk, const CUtensorMap &tm_tv, const CUtensorMap &tm_k_full, const CUtensorMap &tm_k_8, const CUtensorMap &tm_v_full,
                 const CUtensorMap &tm_v_8, cudaStream_t st, int64_t *n_launches);
 
+int launch_policy(const li_policy &pp, int32_t *frame_idx_out, li_policy_result *result, double *partial, cudaStream_t st,
+                  int64_t *n_launches);
+constexpr size_t kPolicyWorkspaceBytes = 1024 * sizeof(double);   // one fp64 partial sum per CTA of li_mse_partial_kernel
+
 }  // namespace li

@@ -30,7 +30,7 @@ def test_every_declared_symbol_is_exported(L):
     assert set(names) == set(li.EXPORTS)
     for n in names:
         assert getattr(L, n) is not None
-    assert li.version() == 100
+    assert li.version() == 101
     assert li.strerror(0) == "ok" and "unsupported" in li.strerror(li.LI_ERR_UNSUPPORTED)
 
 
@@ -151,3 +151,33 @@ def test_missing_library_fails_loudly(monkeypatch, tmp_path):
     monkeypatch.setattr(li, "LIB_PATH", str(tmp_path / "nope.so"))
     with pytest.raises(RuntimeError, match="no CPU fallback"):
         li.lib()
+
+
+def test_context_policy_validation(L):
+    """li_context_policy (Eq. 1-4): host-side argument checks, no launch (pointers are fake device addresses)."""
+    def pol(**over):
+        pp = li.li_policy()
+        pp.z_prev1, pp.z_prev2, pp.n_latent, pp.latent_bf16 = 0x10000, 0x20000, 1000, 0
+        pp.alpha, pp.kappa, pp.L_max, pp.round_nearest = 0.5, 0.02, 8, 0
+        pp.ema_state = 0x30000
+        pp.s_pose, pp.n_cand, pp.tau_pose = 0x40000, 3, 0.45
+        pp.mem_pages, pp.n_mem, pp.win_pages, pp.n_win, pp.cur_pages, pp.n_cur = 0x50000, 2, 0x60000, 20, 0x70000, 4
+        for k, v in over.items():
+            setattr(pp, k, v)
+        return pp
+
+    def call(pp, out=0x80000, cap=14, res=0x90000, ws=0xA0000, ws_bytes=None):
+        n = L.li_policy_workspace_bytes() if ws_bytes is None else ws_bytes
+        return L.li_context_policy(ctypes.byref(pp), out, cap, res, ws, n, None)
+
+    assert L.li_policy_workspace_bytes() == 8192
+    for bad in (dict(z_prev1=0), dict(z_prev2=0x20004), dict(n_latent=0), dict(latent_bf16=2), dict(alpha=0.0),
+                dict(alpha=1.5), dict(kappa=0.0), dict(L_max=0), dict(ema_state=0), dict(s_pose=0), dict(n_cand=-1),
+                dict(mem_pages=0), dict(win_pages=0), dict(cur_pages=0)):
+        assert call(pol(**bad)) == li.LI_ERR_INVALID_ARG, bad
+    assert call(pol(), cap=13) == li.LI_ERR_INVALID_ARG          # capacity < n_mem + min(L_max, n_win) + n_cur
+    assert call(pol(), out=0) == li.LI_ERR_INVALID_ARG
+    assert call(pol(), res=0) == li.LI_ERR_INVALID_ARG
+    assert call(pol(), ws=0) == li.LI_ERR_WORKSPACE
+    assert call(pol(), ws_bytes=100) == li.LI_ERR_WORKSPACE
+    assert call(pol(), ws=0xA0010) == li.LI_ERR_WORKSPACE
