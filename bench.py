@@ -323,6 +323,33 @@ def run_cuda(args):
             extras["attn_ms_identity_contiguous"] = t_ident
             extras["gather_overhead_frac"] = (t_paged - t_ident) / t_ident
             del kc2, vc2, ctx2
+        # li_context_policy (Eq. 1-4, once per chunk): latency at the latent size of one 4-frame chunk of this grid
+        # (16 channels x 4 frames x 60 x 104, bf16), and the streaming MSE against the HBM roofline on 2 x 256 MiB
+        def time_policy(n, reps=12):
+            z1 = torch.randn(n, device=dev).to(torch.bfloat16)
+            z2 = torch.randn(n, device=dev).to(torch.bfloat16)
+            ema = torch.zeros(2, dtype=torch.float32, device=dev)
+            pages = torch.arange(32, dtype=torch.int32, device=dev)
+            out = torch.empty(64, dtype=torch.int32, device=dev)
+            res = torch.zeros(24, dtype=torch.uint8, device=dev)
+            ws = torch.empty(li.lib().li_policy_workspace_bytes(), dtype=torch.uint8, device=dev)
+            sp = torch.rand(8, device=dev)
+            ts = []
+            for _ in range(reps):
+                flush.fill_(7)
+                a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                li.li_context_policy(z1, z2, ema, 0.3, 0.02, 16, sp, 0.45, pages[:4], pages[4:24], pages[24:28], out, res, ws,
+                                     stream=stream)
+                b_.record(stream)
+                torch.cuda.synchronize()
+                ts.append(a.elapsed_time(b_))
+            return float(np.mean(ts[2:]))
+        extras["policy_ms_chunk_latents"] = time_policy(16 * 4 * 60 * 104)
+        n_big = 128 << 20
+        t_big = time_policy(n_big)
+        extras["policy_ms_2x256MiB"] = t_big
+        extras["policy_mse_gbs"] = 2 * n_big * 2 / (t_big * 1e-3) / 1e9
         # sustained load: the board power cap pulls the SM clock down after ~50-100 ms of back-to-back steps, so a long
         # run is slower per step than the short timed region above (MEASURED_PEAKS.json's burst vs sustained figures)
         n_sus = max(50, min(300, int(250.0 / max(float(step_ms.mean()), 1e-3))))

@@ -35,18 +35,23 @@ __global__ void __launch_bounds__(kMseThreads) li_mse_partial_kernel(const void 
   const int64_t n_vec = n / EPV;
   const int64_t stride = (int64_t)gridDim.x * kMseThreads;
   double acc = 0.0;
-  for (int64_t v = (int64_t)blockIdx.x * kMseThreads + threadIdx.x; v < n_vec; v += stride) {
-    const uint4 a = ldg_stream16((const char *)za + v * 16), b = ldg_stream16((const char *)zb + v * 16);
-    float s;
-    if (BF16) {
-      s = (sqdiff_bf16x2(a.x, b.x) + sqdiff_bf16x2(a.y, b.y)) + (sqdiff_bf16x2(a.z, b.z) + sqdiff_bf16x2(a.w, b.w));
-    } else {
-      const float d0 = __uint_as_float(a.x) - __uint_as_float(b.x), d1 = __uint_as_float(a.y) - __uint_as_float(b.y);
-      const float d2 = __uint_as_float(a.z) - __uint_as_float(b.z), d3 = __uint_as_float(a.w) - __uint_as_float(b.w);
-      s = fmaf(d0, d0, d1 * d1) + fmaf(d2, d2, d3 * d3);
+  auto sq = [](const uint4 &a, const uint4 &b) -> float {
+    if (BF16) return (sqdiff_bf16x2(a.x, b.x) + sqdiff_bf16x2(a.y, b.y)) + (sqdiff_bf16x2(a.z, b.z) + sqdiff_bf16x2(a.w, b.w));
+    const float d0 = __uint_as_float(a.x) - __uint_as_float(b.x), d1 = __uint_as_float(a.y) - __uint_as_float(b.y);
+    const float d2 = __uint_as_float(a.z) - __uint_as_float(b.z), d3 = __uint_as_float(a.w) - __uint_as_float(b.w);
+    return fmaf(d0, d0, d1 * d1) + fmaf(d2, d2, d3 * d3);
+  };
+  int64_t v = (int64_t)blockIdx.x * kMseThreads + threadIdx.x;
+  for (; v + 3 * stride < n_vec; v += 4 * stride) {       // 8 independent 16-byte loads in flight per thread
+    uint4 a[4], b[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      a[u] = ldg_stream16((const char *)za + (v + u * stride) * 16);
+      b[u] = ldg_stream16((const char *)zb + (v + u * stride) * 16);
     }
-    acc += (double)s;
+    acc += (double)((sq(a[0], b[0]) + sq(a[1], b[1])) + (sq(a[2], b[2]) + sq(a[3], b[3])));   // one fp64 add per 4 vectors
   }
+  for (; v < n_vec; v += stride) acc += (double)sq(ldg_stream16((const char *)za + v * 16), ldg_stream16((const char *)zb + v * 16));
   if (blockIdx.x == 0 && threadIdx.x < n - n_vec * EPV) {   // ragged tail: fewer than EPV elements
     const int64_t e = n_vec * EPV + threadIdx.x;
     float d;
