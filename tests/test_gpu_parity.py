@@ -271,3 +271,35 @@ def test_tail_wave_split_matches_oracle_and_unsplit_run(P, three_d, monkeypatch)
     assert (buf.o.float().cpu() - o_split).abs().max() <= 4e-3       # one bf16 ulp of |o| <= 0.5
     assert (buf.lse.cpu() - lse_split).abs().max() <= 1e-5
     print(f"small-split: excused={excused} max-abs={mx:.3g} mean-abs={mean:.3g}")
+
+
+def test_tail_wave_split_with_text_and_uneven_calls(P):
+    """Split query blocks in a batch whose calls differ: long history, no history at all (16 half-tiles
+    shared by 5 CTAs: ranges of 3-4), top-k 0; plus a ragged text prefix, so split ranges start inside the text tiles."""
+    import paper_2605_31158_b200 as li
+    from oracle import li_oracle as O
+    spec = W.spec_small(name="small-split-text", H=2, d=128, block=128, frame_tokens=200, n_cur_frames=3, n_pages=72,
+                        n_mem=(6, 0, 3), n_win=(14, 0, 9), density=Fraction(1, 1), pages_per_call=24)
+    prob = W.build(spec)
+    prob.top_k[2] = 0
+    Lt = 333
+    g = torch.Generator().manual_seed(4242)
+    tk = torch.randn((prob.B, spec.H, Lt, spec.d), generator=g).to(torch.bfloat16)
+    tv = torch.randn((prob.B, spec.H, Lt, spec.d), generator=g).to(torch.bfloat16)
+    ctx = li.Context(prob.q.cuda(), prob.k_cache.cuda(), prob.v_cache.cuda(), torch.from_numpy(prob.frame_idx).cuda(),
+                     prob.frame_off, spec.n_cur_frames, spec.block, text_k=tk.cuda(), text_v=tv.cuda())
+    buf = li.Buffers(ctx, prob.kmax, want_scores=True)
+    buf.o.fill_(float("nan"))
+    li.lib().li_reset_launch_count()
+    li.forward(ctx, prob.top_k, buf)
+    torch.cuda.synchronize()
+    assert li.lib().li_launch_count() == 5, "split not taken"
+    osel, osc = P.oracle_select(prob)
+    P.check_selection(prob, buf, osel, osc)
+    gsel = [g_[0] for g_ in P.gpu_selection(prob, buf)]
+    u16 = lambda t: t.contiguous().view(torch.int16).numpy().view(np.uint16)
+    o_ref, lse_ref = O.sparse_attn(prob.u16(prob.q), prob.u16(prob.k_cache), prob.u16(prob.v_cache), prob.frame_idx,
+                                   prob.frame_off, spec.n_cur_frames, spec.block, spec.block, gsel,
+                                   text_k=u16(tk), text_v=u16(tv))
+    mx, mean = P.compare_output(buf.o, buf.lse, o_ref, lse_ref)
+    print(f"small-split-text: max-abs {mx:.3g} mean-abs {mean:.3g}")
