@@ -153,14 +153,18 @@ __device__ __forceinline__ uint32_t order_key(float s) {
   return (u & 0x80000000u) ? ~u : (u | 0x80000000u);   // unsigned order == float order
 }
 
-// Scores (Eq. 10).  grid = (ceil(Mmax/32), ceil(Nqb/8), B*H), ONE warp per CTA (thousands of independent warps:
-// the work is latency-bound, so it is spread as thinly as possible).  lane = one historical block m; the lane walks
-// its pooled key row (16-byte read-only loads) against 8 pooled query rows broadcast from shared memory: 8
-// independent fp32 FMA chains, no cross-lane reduction.  Output: order-preserving keys [B,H,Nqb,Mmax] (+ scores).
+// Scores (Eq. 10).  grid = (ceil(Mmax/32), ceil(Nqb/8), B*H), 4 warps per CTA.  The work is latency-bound (a few MFLOP
+// spread over thousands of CTAs), so the dependent chain of every warp is kept short: lane = one historical block m,
+// warp w walks channels [w*D/4, (w+1)*D/4) of its pooled key row (one coalesced 128-byte line per channel, kbar is
+// channel-major) against 8 pooled query rows broadcast from shared memory = 8 independent fp32 FMA chains; the 4
+// partial sums of a score are added in a fixed order (w = 0..3) through shared memory.  Output: order-preserving keys
+// [B,H,Nqb,Mmax] (+ scores).
+constexpr int kScoreWarps = 4;
 template <int D>
-__global__ void __launch_bounds__(32) li_score_kernel(const SelectParams p, const BatchMeta meta) {
+__global__ void __launch_bounds__(kScoreWarps * 32) li_score_kernel(const SelectParams p, const BatchMeta meta) {
   __shared__ __align__(16) float sq[kRowsPerWarp * D];
-  const int lane = threadIdx.x;
+  __shared__ float part[kScoreWarps][kRowsPerWarp][32];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int bh = blockIdx.z, b = bh / p.H;
   const int i0 = blockIdx.y * kRowsPerWarp;
   const int n_hist = meta.frame_off[b + 1] - meta.frame_off[b] - p.n_cur;
@@ -172,50 +176,44 @@ __global__ void __launch_bounds__(32) li_score_kernel(const SelectParams p, cons
 
   // kbar is [B,H,d,Mp] (written transposed by the pool kernel): for a fixed channel the 32 lanes read 32
   // consecutive floats = one 128-byte line.  Lanes past M read padding and their results are dropped.
-  const float *kT = p.kbar + (int64_t)bh * D * p.Mp + m;
+  constexpr int DW = D / kScoreWarps;                        // channels per warp
   constexpr int CH = 16;                                     // channels per batch of loads
-  float kv[CH];
+  const float *kT = p.kbar + ((int64_t)bh * D + warp * DW) * p.Mp + m;
+  float kv[DW];
 #pragma unroll
-  for (int c = 0; c < CH; ++c) kv[c] = __ldg(kT + (int64_t)c * p.Mp);   // in flight while the q rows are staged
-  for (int t = lane; t < kRowsPerWarp * D / 4; t += 32) {
+  for (int c = 0; c < DW; ++c) kv[c] = __ldg(kT + (int64_t)c * p.Mp);   // all in flight while the q rows are staged
+  for (int t = threadIdx.x; t < kRowsPerWarp * D / 4; t += kScoreWarps * 32) {
     const int g = t / (D / 4);
     reinterpret_cast<float4 *>(sq)[t] =
         (i0 + g < p.Nqb) ? __ldg(reinterpret_cast<const float4 *>(p.qbar + ((int64_t)bh * p.Nqb + i0) * D) + t)
                          : make_float4(0.f, 0.f, 0.f, 0.f);
   }
-  __syncwarp();
+  __syncthreads();
 
   float acc[kRowsPerWarp];
 #pragma unroll
   for (int g = 0; g < kRowsPerWarp; ++g) acc[g] = 0.f;
 #pragma unroll
-  for (int c0 = 0; c0 < D; c0 += CH) {
-    float nx[CH];
-    if (c0 + CH < D) {
-#pragma unroll
-      for (int c = 0; c < CH; ++c) nx[c] = __ldg(kT + (int64_t)(c0 + CH + c) * p.Mp);
-    }
-#pragma unroll
-    for (int c = 0; c < CH; c += 4) {
-#pragma unroll
-      for (int g = 0; g < kRowsPerWarp; ++g) {
-        const float4 qv = *reinterpret_cast<const float4 *>(sq + g * D + c0 + c);
-        acc[g] = fmaf(qv.x, kv[c], acc[g]);
-        acc[g] = fmaf(qv.y, kv[c + 1], acc[g]);
-        acc[g] = fmaf(qv.z, kv[c + 2], acc[g]);
-        acc[g] = fmaf(qv.w, kv[c + 3], acc[g]);
-      }
-    }
-    if (c0 + CH < D) {
-#pragma unroll
-      for (int c = 0; c < CH; ++c) kv[c] = nx[c];
-    }
-  }
-  if (m < M) {
+  for (int c = 0; c < DW; c += 4) {
 #pragma unroll
     for (int g = 0; g < kRowsPerWarp; ++g) {
+      const float4 qv = *reinterpret_cast<const float4 *>(sq + g * D + warp * DW + c);
+      acc[g] = fmaf(qv.x, kv[c], acc[g]);
+      acc[g] = fmaf(qv.y, kv[c + 1], acc[g]);
+      acc[g] = fmaf(qv.z, kv[c + 2], acc[g]);
+      acc[g] = fmaf(qv.w, kv[c + 3], acc[g]);
+    }
+  }
+#pragma unroll
+  for (int g = 0; g < kRowsPerWarp; ++g) part[warp][g][lane] = acc[g];
+  __syncthreads();
+  if (m < M) {
+#pragma unroll
+    for (int gg = 0; gg < kRowsPerWarp / kScoreWarps; ++gg) {     // warp w finishes rows w*2, w*2+1
+      const int g = warp * (kRowsPerWarp / kScoreWarps) + gg;
       if (i0 + g < p.Nqb) {
-        const float sc = acc[g] * p.inv_sqrt_d + 0.0f;       // -0 -> +0 so that equal scores have equal keys
+        const float dot = ((part[0][g][lane] + part[1][g][lane]) + part[2][g][lane]) + part[3][g][lane];
+        const float sc = dot * p.inv_sqrt_d + 0.0f;          // -0 -> +0 so that equal scores have equal keys
         p.keys[((int64_t)bh * p.Nqb + i0 + g) * p.Mmax + m] = order_key(sc);
         if (p.scores != nullptr) p.scores[((int64_t)bh * p.Nqb + i0 + g) * p.score_pitch + m] = sc;
       }
@@ -324,7 +322,7 @@ int launch_select(const SelectParams &sp, const BatchMeta &meta, cudaStream_t st
   if (sp.Mmax > 0) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((sp.Mmax + 31) / 32, (sp.Nqb + kRowsPerWarp - 1) / kRowsPerWarp, sp.B * sp.H);
-    cfg.blockDim = dim3(32);
+    cfg.blockDim = dim3(kScoreWarps * 32);
     cfg.stream = st;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
