@@ -102,3 +102,32 @@ def test_text_prefix_is_always_attended(P, mode, Lt):
                                        text_k=u16(tk), text_v=u16(tv))
     mx, mean = P.compare_output(buf.o, buf.lse, o_ref, lse_ref)
     print(f"text {mode} Lt={Lt}: max-abs {mx:.3g} mean-abs {mean:.3g}")
+
+
+def test_3d_more_tiles_than_the_shared_memory_tables_hold(P):
+    """One query block attending 2150 selected 3-D blocks (+1 chunk block): more tiles than the per-CTA geometry table
+    (2048), the selected-index table (1024) and the frame table (256) hold, so the global-memory fallbacks run; the
+    single query block is also shared by 8 CTAs (tail-wave split).  Pages repeat, so ties are exact: bit-identical mask."""
+    import paper_2605_31158_b200 as li
+    from oracle import li_oracle as O
+    g = torch.Generator().manual_seed(23)
+    H, d, gh, gw, bt, bh, bw = 1, 64, 8, 4, 4, 8, 4
+    T_f, n_hist, k = gh * gw, 4 * 2200, 2150
+    q = torch.randn((1, H, 4 * T_f, d), generator=g).to(torch.bfloat16)
+    kc = torch.randn((12, H, T_f, d), generator=g).to(torch.bfloat16)
+    vc = torch.randn((12, H, T_f, d), generator=g).to(torch.bfloat16)
+    fi = np.concatenate([torch.randint(0, 8, (n_hist,), generator=g).numpy(), [8, 9, 10, 11]]).astype(np.int32)
+    fo = np.asarray([0, n_hist + 4], np.int32)
+    ctx = li.Context(q.cuda(), kc.cuda(), vc.cuda(), torch.from_numpy(fi).cuda(), fo, 4, 128, grid=(gh, gw),
+                     block3d=(bt, bh, bw))
+    assert ctx.Nqb == 1 and ctx.Mmax == 2200
+    buf = li.Buffers(ctx, k, want_scores=True)
+    li.lib().li_reset_launch_count()
+    li.forward(ctx, [k], buf)
+    torch.cuda.synchronize()
+    assert li.lib().li_launch_count() == 5
+    u16 = lambda t: t.view(torch.int16).numpy().view(np.uint16)
+    osel, osc = O.block_select_3d(u16(q), u16(kc), fi, fo, 4, gh, gw, bt, bh, bw, [k])
+    np.testing.assert_array_equal(buf.sel_idx.cpu().numpy()[0], osel[0])
+    o_ref, lse_ref = O.sparse_attn_3d(u16(q), u16(kc), u16(vc), fi, fo, 4, gh, gw, bt, bh, bw, osel)
+    P.compare_output(buf.o, buf.lse, o_ref, lse_ref)
