@@ -303,3 +303,29 @@ def test_tail_wave_split_with_text_and_uneven_calls(P):
                                    text_k=u16(tk), text_v=u16(tv))
     mx, mean = P.compare_output(buf.o, buf.lse, o_ref, lse_ref)
     print(f"small-split-text: max-abs {mx:.3g} mean-abs {mean:.3g}")
+
+
+def test_whole_step_is_cuda_graph_capturable(P):
+    """li_block_select + li_sparse_attn (4 launches with programmatic dependencies, here 5 with the split's merge) issue
+    no synchronising call, so a step can be captured once and replayed; the replay must reproduce the eager outputs
+    bit for bit, also after the inputs changed in place."""
+    import paper_2605_31158_b200 as li
+    spec = W.spec_small(name="small-graph", H=2, d=128, block=128, frame_tokens=200, n_cur_frames=3, n_pages=24,
+                        n_mem=(6,), n_win=(14,), density=Fraction(1, 2))
+    prob = W.build(spec)
+    ctx, buf = P.run_gpu(prob, want_scores=False)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=side):
+        li.forward(ctx, prob.top_k, buf, stream=side)
+    for seed in (1, 2):
+        g = torch.Generator().manual_seed(seed)
+        ctx.q.copy_(torch.randn(prob.q.shape, generator=g).to(torch.bfloat16))    # new queries, same buffers
+        li.forward(ctx, prob.top_k, buf)
+        torch.cuda.synchronize()
+        sel, o, lse = buf.sel_idx.clone(), buf.o.clone(), buf.lse.clone()
+        buf.sel_idx.fill_(-9); buf.o.zero_(); buf.lse.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(buf.sel_idx, sel) and torch.equal(buf.o, o) and torch.equal(buf.lse, lse)
