@@ -36,7 +36,7 @@
 extern "C" {
 #endif
 
-#define LI_VERSION 101          /* major*100 + minor */
+#define LI_VERSION 102          /* major*100 + minor */
 #define LI_MAX_CALLS 64         /* max B per call of the library (batch of independent attention calls) */
 
 enum {
@@ -102,6 +102,21 @@ int li_block_select(const li_problem *p, const int32_t *top_k_host, int32_t kmax
 int li_block_select_reuse_kbar(const li_problem *p, const int32_t *top_k_host, int32_t kmax,
                                int32_t *sel_idx, int32_t *sel_cnt, float *scores_opt, int32_t score_pitch,
                                void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* Page-resident pooled slices (3-D tiling only; LI_ERR_UNSUPPORTED otherwise).  A 3-D block is bt frames
+ * x one bh x bw patch of the frame grid, and the sum of a frame's K rows over a patch does not depend on where the frame
+ * sits in a call's frame list.  li_pool_pages computes these sums for the listed pages (call it for a page whenever its
+ * K rows were written: once per chunk for the chunk's pages) into
+ *   slice_cache : fp32 [n_pages][H][Hb*Wb][d], li_slice_cache_bytes(p) bytes, 16-byte aligned, owned by the caller;
+ * li_block_select_cached is li_block_select with the pooled historical keys (Eq. 9) formed from <= bt cached rows per
+ * block instead of the block's 128 K rows: it reads Lq*d*2*H + M*bt*d*4*H bytes instead of (Lq + L_hist)*d*2*H.  Same
+ * means up to the fp32 summation order (patch sums first), same scores / top-k semantics.  Every page of the history
+ * must have been pooled since it was last written (not checked).  pages_dev: DEVICE int32 [n_list]. */
+size_t li_slice_cache_bytes(const li_problem *p);
+int li_pool_pages(const li_problem *p, const int32_t *pages_dev, int32_t n_list, float *slice_cache, void *cuda_stream);
+int li_block_select_cached(const li_problem *p, const int32_t *top_k_host, int32_t kmax,
+                           int32_t *sel_idx, int32_t *sel_cnt, float *scores_opt, int32_t score_pitch,
+                           const float *slice_cache, void *workspace, size_t workspace_bytes, void *cuda_stream);
 
 /* Eq. 11 + attention.  Query block i of (b,h) attends ALL text tokens (if any), ALL chunk tokens
  * (bidirectional inside the chunk) plus the valid tokens of historical blocks sel_idx[b,h,i,0..sel_cnt[b,h,i]); the same

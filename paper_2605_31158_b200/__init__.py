@@ -19,7 +19,8 @@ LIB_PATH = os.path.join(_HERE, "libli.so")
 LI_OK, LI_ERR_INVALID_ARG, LI_ERR_UNSUPPORTED, LI_ERR_WORKSPACE, LI_ERR_CUDA = 0, -1, -2, -3, -4
 LI_MAX_CALLS = 64
 
-EXPORTS = ("li_block_select", "li_block_select_reuse_kbar", "li_sparse_attn", "li_workspace_bytes", "li_context_policy",
+EXPORTS = ("li_block_select", "li_block_select_reuse_kbar", "li_block_select_cached", "li_pool_pages", "li_slice_cache_bytes",
+           "li_sparse_attn", "li_workspace_bytes", "li_context_policy",
            "li_policy_workspace_bytes", "li_launch_count", "li_reset_launch_count", "li_strerror", "li_version")
 
 
@@ -89,6 +90,14 @@ def lib() -> ctypes.CDLL:
         L.li_sparse_attn.restype = ctypes.c_int
         L.li_sparse_attn.argtypes = [P, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p,
                                      ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p]
+        L.li_slice_cache_bytes.restype = ctypes.c_size_t
+        L.li_slice_cache_bytes.argtypes = [P]
+        L.li_pool_pages.restype = ctypes.c_int
+        L.li_pool_pages.argtypes = [P, ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p, ctypes.c_void_p]
+        L.li_block_select_cached.restype = ctypes.c_int
+        L.li_block_select_cached.argtypes = [P, ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p, ctypes.c_void_p,
+                                             ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p, ctypes.c_void_p,
+                                             ctypes.c_size_t, ctypes.c_void_p]
         L.li_policy_workspace_bytes.restype = ctypes.c_size_t
         L.li_policy_workspace_bytes.argtypes = []
         L.li_context_policy.restype = ctypes.c_int
@@ -206,6 +215,39 @@ def li_block_select(ctx: Context, top_k: Sequence[int], kmax: int, sel_idx: torc
                                _stream_ptr(stream))
     if rc != LI_OK:
         raise LiError(rc, "li_block_select")
+
+
+def li_slice_cache_bytes(ctx: Context) -> int:
+    return int(lib().li_slice_cache_bytes(ctypes.byref(ctx.p)))
+
+
+def li_pool_pages(ctx: Context, pages: torch.Tensor, slice_cache: torch.Tensor,
+                  stream: Optional[torch.cuda.Stream] = None) -> None:
+    """li_pool_pages (include/li.h): patch sums of the listed K pages (int32 CUDA tensor) into slice_cache (fp32 CUDA
+    tensor of li_slice_cache_bytes bytes).  3-D tiling only."""
+    if pages.dtype != torch.int32 or not pages.is_cuda or not pages.is_contiguous():
+        raise ValueError("pages must be a contiguous int32 CUDA tensor")
+    if slice_cache.dtype != torch.float32 or not slice_cache.is_cuda or not slice_cache.is_contiguous() or \
+            slice_cache.numel() * 4 < li_slice_cache_bytes(ctx):
+        raise ValueError("slice_cache must be a contiguous fp32 CUDA tensor of li_slice_cache_bytes bytes")
+    rc = lib().li_pool_pages(ctypes.byref(ctx.p), pages.data_ptr(), pages.numel(), slice_cache.data_ptr(), _stream_ptr(stream))
+    if rc != LI_OK:
+        raise LiError(rc, "li_pool_pages")
+
+
+def li_block_select_cached(ctx: Context, top_k: Sequence[int], kmax: int, sel_idx: torch.Tensor, sel_cnt: torch.Tensor,
+                           slice_cache: torch.Tensor, workspace: torch.Tensor, scores: Optional[torch.Tensor] = None,
+                           stream: Optional[torch.cuda.Stream] = None) -> None:
+    """li_block_select_cached (include/li.h): li_block_select with the historical block means formed from slice_cache."""
+    tk = np.ascontiguousarray(np.asarray(top_k, dtype=np.int32))
+    if len(tk) != ctx.B:
+        raise ValueError("top_k must have B entries")
+    pitch = int(scores.shape[-1]) if scores is not None else 0
+    rc = lib().li_block_select_cached(ctypes.byref(ctx.p), tk.ctypes.data, int(kmax), sel_idx.data_ptr(), sel_cnt.data_ptr(),
+                                      scores.data_ptr() if scores is not None else None, pitch, slice_cache.data_ptr(),
+                                      workspace.data_ptr(), workspace.numel() * workspace.element_size(), _stream_ptr(stream))
+    if rc != LI_OK:
+        raise LiError(rc, "li_block_select_cached")
 
 
 def li_sparse_attn(ctx: Context, sel_idx: torch.Tensor, sel_cnt: torch.Tensor, kmax: int, o: torch.Tensor,

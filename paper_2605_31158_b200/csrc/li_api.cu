@@ -153,10 +153,11 @@ size_t li_workspace_bytes(const li_problem *p, int32_t kmax) {
 
 static int block_select_impl(const li_problem *p, const int32_t *top_k_host, int32_t kmax, int32_t *sel_idx,
                              int32_t *sel_cnt, float *scores_opt, int32_t score_pitch, void *workspace,
-                             size_t workspace_bytes, void *cuda_stream, int skip_k) {
+                             size_t workspace_bytes, void *cuda_stream, int skip_k, const float *slice_cache = nullptr) {
   Derived dv;
   int rc = check_problem(p, &dv);
   if (rc != LI_OK) return rc;
+  if (slice_cache != nullptr && dv.tl.bt == 0) return LI_ERR_UNSUPPORTED;   // patch sums exist for 3-D blocks only
   if (top_k_host == nullptr || sel_idx == nullptr || sel_cnt == nullptr || kmax < 1) return LI_ERR_INVALID_ARG;
   if (scores_opt != nullptr && score_pitch < dv.Mmax) return LI_ERR_INVALID_ARG;
   if (workspace == nullptr || workspace_bytes < ws_bytes(p, dv) + ws_split_bytes(p) || ((uintptr_t)workspace & 255u))
@@ -187,9 +188,46 @@ static int block_select_impl(const li_problem *p, const int32_t *top_k_host, int
   sp.sel_idx = sel_idx; sp.sel_cnt = sel_cnt; sp.scores = scores_opt;
   sp.inv_sqrt_d = 1.0f / std::sqrt((float)p->d);
   int64_t n = 0;
-  const int e = li::launch_select(sp, dv.meta, (cudaStream_t)cuda_stream, &n);
+  int e = 0;
+  if (slice_cache != nullptr) {             // kbar from the cached patch sums; the pool kernel then handles Q only
+    e = li::launch_kbar_from_slices(sp, dv.meta, slice_cache, (cudaStream_t)cuda_stream, &n);
+    sp.skip_k = 1;
+  }
+  if (e == 0) e = li::launch_select(sp, dv.meta, (cudaStream_t)cuda_stream, &n);
   g_launches += n;
   return e == 0 ? LI_OK : LI_ERR_CUDA;
+}
+
+size_t li_slice_cache_bytes(const li_problem *p) {
+  Derived dv;
+  if (check_problem(p, &dv) != LI_OK || dv.tl.bt == 0) return 0;
+  return (size_t)p->n_pages * p->H * dv.tl.Hb * dv.tl.Wb * p->d * 4;
+}
+
+int li_pool_pages(const li_problem *p, const int32_t *pages_dev, int32_t n_list, float *slice_cache, void *cuda_stream) {
+  Derived dv;
+  int rc = check_problem(p, &dv);
+  if (rc != LI_OK) return rc;
+  if (dv.tl.bt == 0) return LI_ERR_UNSUPPORTED;
+  if (n_list < 0 || slice_cache == nullptr || (n_list > 0 && pages_dev == nullptr) || ((uintptr_t)slice_cache & 15u))
+    return LI_ERR_INVALID_ARG;
+  li::SelectParams sp;
+  std::memset(&sp, 0, sizeof(sp));
+  sp.tl = dv.tl;
+  sp.H = p->H; sp.d = p->d;
+  sp.k_cache = (const uint16_t *)p->k_cache; sp.kv_sp = p->kv_sp; sp.kv_sh = p->kv_sh; sp.kv_st = p->kv_st;
+  int64_t n = 0;
+  const int e = li::launch_pool_pages(sp, pages_dev, n_list, slice_cache, (cudaStream_t)cuda_stream, &n);
+  g_launches += n;
+  return e == 0 ? LI_OK : LI_ERR_CUDA;
+}
+
+int li_block_select_cached(const li_problem *p, const int32_t *top_k_host, int32_t kmax, int32_t *sel_idx,
+                           int32_t *sel_cnt, float *scores_opt, int32_t score_pitch, const float *slice_cache,
+                           void *workspace, size_t workspace_bytes, void *cuda_stream) {
+  if (slice_cache == nullptr) return LI_ERR_INVALID_ARG;
+  return block_select_impl(p, top_k_host, kmax, sel_idx, sel_cnt, scores_opt, score_pitch, workspace, workspace_bytes,
+                           cuda_stream, 0, slice_cache);
 }
 
 int li_block_select(const li_problem *p, const int32_t *top_k_host, int32_t kmax, int32_t *sel_idx, int32_t *sel_cnt,

@@ -177,7 +177,6 @@ __global__ void __launch_bounds__(kScoreWarps * 32) li_score_kernel(const Select
   // kbar is [B,H,d,Mp] (written transposed by the pool kernel): for a fixed channel the 32 lanes read 32
   // consecutive floats = one 128-byte line.  Lanes past M read padding and their results are dropped.
   constexpr int DW = D / kScoreWarps;                        // channels per warp
-  constexpr int CH = 16;                                     // channels per batch of loads
   const float *kT = p.kbar + ((int64_t)bh * D + warp * DW) * p.Mp + m;
   float kv[DW];
 #pragma unroll
@@ -300,6 +299,75 @@ __global__ void __launch_bounds__(kTopkWarps * 32) li_topk_kernel(const SelectPa
     }
   }
   for (int t = k + lane; t < p.kmax; t += 32) out[t] = -1;
+}
+
+// ----------------------------------------------------------------------------- page-resident pooled slices
+// 3-D tiling only.  A 3-D block is bt frames x one bh x bw patch, and a frame's patch sum does not depend on
+// where the frame sits in a call's logical list, so it is computed ONCE when the page is written:
+//   cache [n_pages][H][Hb*Wb][D] fp32 = sum of the K rows of that frame's patch (rows inside the grid only).
+// Selection then pools a historical block from <= bt cached rows instead of 128 K rows (1/32 of the bytes).
+template <int D>
+__global__ void __launch_bounds__(128) li_pool_pages_kernel(const SelectParams p, const int32_t *pages, float *cache) {
+  constexpr int TPR = D / 8;                 // threads per row (16-byte loads)
+  constexpr int RPP = 128 / TPR;             // rows per pass
+  __shared__ float red[RPP][D];
+  const Tiling tl = p.tl;
+  const int patch = blockIdx.x, h = blockIdx.y, page = pages[blockIdx.z];
+  const int hb = patch / tl.Wb, wb = patch - hb * tl.Wb;
+  const int r0 = threadIdx.x / TPR, cofs = (threadIdx.x % TPR) * 8;
+  float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  const uint16_t *base = p.k_cache + (int64_t)page * p.kv_sp + h * p.kv_sh + cofs;
+#pragma unroll
+  for (int it = 0; it < 32 / RPP; ++it) {
+    const int r = r0 + it * RPP, hh = r / tl.bw, ww = r - hh * tl.bw, y = hb * tl.bh + hh;
+    if (y < tl.gh) add_bf16x8(acc, ldg_stream(base + (int64_t)(y * tl.gw + wb * tl.bw + ww) * p.kv_st));
+  }
+#pragma unroll
+  for (int e = 0; e < 8; ++e) red[r0][cofs + e] = acc[e];
+  __syncthreads();
+  if (threadIdx.x < D) {
+    float s = 0.f;
+#pragma unroll
+    for (int r = 0; r < RPP; ++r) s += red[r][threadIdx.x];
+    cache[(((int64_t)page * p.H + h) * (tl.Hb * tl.Wb) + patch) * D + threadIdx.x] = s;
+  }
+}
+
+// kbar of every historical block from the cached patch sums of its frames.  grid (Mmax, H, B), D threads = channels.
+template <int D>
+__global__ void __launch_bounds__(D) li_kbar_from_slices_kernel(const SelectParams p, const BatchMeta meta, const float *cache) {
+  const Tiling tl = p.tl;
+  const int m = blockIdx.x, h = blockIdx.y, b = blockIdx.z, c = threadIdx.x;
+  const int foff = meta.frame_off[b];
+  const int n_hist = meta.frame_off[b + 1] - foff - p.n_cur;
+  if (m >= tl.num_blocks(n_hist, p.T_f, p.blk)) return;
+  const int per = tl.Hb * tl.Wb, tg = m / per, patch = m - tg * per, hb = patch / tl.Wb;
+  const int nf = min(tl.bt, n_hist - tg * tl.bt);
+  float s = 0.f;
+  for (int f = 0; f < nf; ++f) {
+    const int page = __ldg(p.frame_idx + foff + tg * tl.bt + f);
+    s += __ldg(cache + (((int64_t)page * p.H + h) * per + patch) * D + c);
+  }
+  const int nvalid = nf * min(tl.bh, tl.gh - hb * tl.bh) * tl.bw;                    // Eq. 9: true cardinality |K_m|
+  p.kbar[(((int64_t)b * p.H + h) * D + c) * p.Mp + m] = s / (float)nvalid;         // kbar is [B,H,d,Mp]
+}
+
+int launch_pool_pages(const SelectParams &sp, const int32_t *pages, int n_list, float *cache, cudaStream_t st, int64_t *n_launches) {
+  if (n_list <= 0) return 0;
+  dim3 grid(sp.tl.Hb * sp.tl.Wb, sp.H, n_list);
+  if (sp.d == 128) li_pool_pages_kernel<128><<<grid, 128, 0, st>>>(sp, pages, cache);
+  else li_pool_pages_kernel<64><<<grid, 128, 0, st>>>(sp, pages, cache);
+  if (n_launches) *n_launches += 1;
+  return (int)cudaGetLastError();
+}
+
+int launch_kbar_from_slices(const SelectParams &sp, const BatchMeta &meta, const float *cache, cudaStream_t st, int64_t *n_launches) {
+  if (sp.Mmax <= 0) return 0;
+  dim3 grid(sp.Mmax, sp.H, sp.B);
+  if (sp.d == 128) li_kbar_from_slices_kernel<128><<<grid, 128, 0, st>>>(sp, meta, cache);
+  else li_kbar_from_slices_kernel<64><<<grid, 64, 0, st>>>(sp, meta, cache);
+  if (n_launches) *n_launches += 1;
+  return (int)cudaGetLastError();
 }
 
 int launch_select(const SelectParams &sp, const BatchMeta &meta, cudaStream_t st, int64_t *n_launches) {

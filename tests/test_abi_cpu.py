@@ -30,7 +30,7 @@ def test_every_declared_symbol_is_exported(L):
     assert set(names) == set(li.EXPORTS)
     for n in names:
         assert getattr(L, n) is not None
-    assert li.version() == 101
+    assert li.version() == 102
     assert li.strerror(0) == "ok" and "unsupported" in li.strerror(li.LI_ERR_UNSUPPORTED)
 
 
@@ -181,3 +181,26 @@ def test_context_policy_validation(L):
     assert call(pol(), ws=0) == li.LI_ERR_WORKSPACE
     assert call(pol(), ws_bytes=100) == li.LI_ERR_WORKSPACE
     assert call(pol(), ws=0xA0010) == li.LI_ERR_WORKSPACE
+
+
+def test_slice_cache_validation(L):
+    """li_pool_pages / li_block_select_cached exist for the 3-D tiling only; host-side argument checks."""
+    p1, keep1 = make_problem()                       # 1-D blocks
+    assert L.li_slice_cache_bytes(ctypes.byref(p1)) == 0
+    assert L.li_pool_pages(ctypes.byref(p1), 0x50000, 1, 0x60000, None) == li.LI_ERR_UNSUPPORTED
+    tk = np.asarray([8], dtype=np.int32)
+    ws = L.li_workspace_bytes(ctypes.byref(p1), 8)
+    assert L.li_block_select_cached(ctypes.byref(p1), tk.ctypes.data, 8, 0x60000, 0x70000, None, 0, 0x90000, 0x50000, ws,
+                                    None) == li.LI_ERR_UNSUPPORTED
+    fo = np.asarray([0, 6], dtype=np.int32)
+    p3, keep3 = make_problem(frame_tokens=30 * 52, Lq=2 * 30 * 52, d=128, block_q=128, block_k=128, n_cur_frames=2,
+                             q_sb=24 * 3120 * 128, q_sh=3120 * 128, q_st=128, kv_sp=24 * 1560 * 128, kv_sh=1560 * 128,
+                             kv_st=128, H=24, grid_h=30, grid_w=52, bt=4, bh=8, bw=4)
+    p3.frame_off_host = fo.ctypes.data
+    assert L.li_slice_cache_bytes(ctypes.byref(p3)) == p3.n_pages * 24 * 4 * 13 * 128 * 4
+    assert L.li_pool_pages(ctypes.byref(p3), 0, 1, 0x60000, None) == li.LI_ERR_INVALID_ARG
+    assert L.li_pool_pages(ctypes.byref(p3), 0x50000, 1, 0, None) == li.LI_ERR_INVALID_ARG
+    assert L.li_pool_pages(ctypes.byref(p3), 0x50000, -1, 0x60000, None) == li.LI_ERR_INVALID_ARG
+    ws3 = L.li_workspace_bytes(ctypes.byref(p3), 8)
+    assert L.li_block_select_cached(ctypes.byref(p3), tk.ctypes.data, 8, 0x60000, 0x70000, None, 0, 0, 0x50000, ws3,
+                                    None) == li.LI_ERR_INVALID_ARG

@@ -131,3 +131,41 @@ def test_3d_more_tiles_than_the_shared_memory_tables_hold(P):
     np.testing.assert_array_equal(buf.sel_idx.cpu().numpy()[0], osel[0])
     o_ref, lse_ref = O.sparse_attn_3d(u16(q), u16(kc), u16(vc), fi, fo, 4, gh, gw, bt, bh, bw, osel)
     P.compare_output(buf.o, buf.lse, o_ref, lse_ref)
+
+
+@pytest.mark.parametrize("grid,block3d,n_cur,n_hist,d", [((30, 52), (4, 8, 4), 4, (2, 4), 128),   # paper geometry, border patches
+                                                          ((10, 16), (4, 4, 8), 4, (3, 3), 128),   # (4,4,8), partial group
+                                                          ((12, 8), (2, 8, 4), 2, (2, 3), 64),     # 64-token blocks, d = 64
+                                                          ((6, 8), (4, 8, 4), 3, (1, 4), 128)])    # grid lower than a patch
+def test_select_from_page_resident_patch_sums(P, grid, block3d, n_cur, n_hist, d):
+    """li_pool_pages + li_block_select_cached (include/li.h): historical block means formed from per-page patch sums
+    must give the oracle's scores and mask, also after a page was rewritten and re-pooled alone, and for a batch of
+    calls sharing the page pool."""
+    import paper_2605_31158_b200 as li
+    spec = small3d(f"s3d-cache-{grid}-{block3d}", grid, block3d, n_cur, (n_hist[0], 0, 1), (n_hist[1], 2, 3), d=d,
+                   n_pages=42, pages_per_call=14)
+    prob = W.build(spec)
+    ctx = P.upload(prob)
+    buf = li.Buffers(ctx, prob.kmax, want_scores=True)
+    cache = torch.full((li.li_slice_cache_bytes(ctx) // 4,), float("nan"), dtype=torch.float32, device="cuda")
+    li.li_pool_pages(ctx, torch.arange(spec.n_pages, dtype=torch.int32, device="cuda"), cache)
+    for rewrite in (False, True):
+        if rewrite:          # the model rewrites one historical page of call 0: only that page is pooled again
+            pg = int(prob.frame_idx[0])
+            g = torch.Generator().manual_seed(99)
+            prob.k_cache[pg] = torch.randn(prob.k_cache[pg].shape, generator=g).to(torch.bfloat16)
+            ctx.k_cache[pg].copy_(prob.k_cache[pg])
+            li.li_pool_pages(ctx, torch.tensor([pg], dtype=torch.int32, device="cuda"), cache)
+        buf.sel_idx.fill_(-7)
+        li.li_block_select_cached(ctx, prob.top_k, buf.kmax, buf.sel_idx, buf.sel_cnt, cache, buf.workspace, buf.scores)
+        torch.cuda.synchronize()
+        osel, osc = P.oracle_select(prob)
+        excused = P.check_selection(prob, buf, osel, osc)
+        # and the direct path on the same data: same scores up to the fp32 summation order
+        sc_cached = buf.scores.clone()
+        li.li_block_select(ctx, prob.top_k, buf.kmax, buf.sel_idx, buf.sel_cnt, buf.workspace, buf.scores)
+        torch.cuda.synchronize()
+        for b in range(prob.B):
+            M = prob.M(b)
+            torch.testing.assert_close(sc_cached[b, :, :, :M], buf.scores[b, :, :, :M], rtol=1e-5, atol=1e-6)
+    print(f"cached select {grid} {block3d}: excused={excused}")
