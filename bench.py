@@ -374,6 +374,27 @@ def run_cuda(args):
             torch.cuda.synchronize()
             ts.append(a.elapsed_time(b_))
         extras["select_ms_reuse_kbar"] = float(np.mean(ts[2:]))
+        if s.grid is not None:
+            # 3-D tiling: select from page-resident patch sums (li_pool_pages once per written page, then
+            # li_block_select_cached); the chunk's pages are the ones (re)pooled every step
+            cache = torch.empty(li.li_slice_cache_bytes(ctx) // 4, dtype=torch.float32, device=dev)
+            li.li_pool_pages(ctx, torch.arange(s.n_pages, dtype=torch.int32, device=dev), cache, stream)
+            cur_t = torch.tensor(cur_pages, dtype=torch.int32, device=dev)
+            t_sel, t_pool = [], []
+            for _ in range(12):
+                flush.fill_(6)
+                a, b_, c_ = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+                a.record(stream)
+                li.li_pool_pages(ctx, cur_t, cache, stream)
+                b_.record(stream)
+                li.li_block_select_cached(ctx, prob.top_k, buf.kmax, buf.sel_idx, buf.sel_cnt, cache, buf.workspace, None, stream)
+                c_.record(stream)
+                torch.cuda.synchronize()
+                t_pool.append(a.elapsed_time(b_)); t_sel.append(b_.elapsed_time(c_))
+            extras["pool_pages_ms_chunk"] = float(np.mean(t_pool[2:]))
+            extras["select_ms_slice_cache"] = float(np.mean(t_sel[2:]))
+            li.li_block_select(ctx, prob.top_k, buf.kmax, buf.sel_idx, buf.sel_cnt, buf.workspace, None, stream)
+            del cache
         order = torch.from_numpy(prob.frame_idx.astype(np.int64)).to(dev)
         free_b = torch.cuda.mem_get_info()[0]
         need_b = 2 * order.numel() * kc[0].numel() * 2

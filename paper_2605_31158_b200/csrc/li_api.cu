@@ -189,11 +189,8 @@ static int block_select_impl(const li_problem *p, const int32_t *top_k_host, int
   sp.inv_sqrt_d = 1.0f / std::sqrt((float)p->d);
   int64_t n = 0;
   int e = 0;
-  if (slice_cache != nullptr) {             // kbar from the cached patch sums; the pool kernel then handles Q only
-    e = li::launch_kbar_from_slices(sp, dv.meta, slice_cache, (cudaStream_t)cuda_stream, &n);
-    sp.skip_k = 1;
-  }
-  if (e == 0) e = li::launch_select(sp, dv.meta, (cudaStream_t)cuda_stream, &n);
+  sp.slice_cache = slice_cache;             // non-null: the pool kernel forms kbar from the cached patch sums
+  e = li::launch_select(sp, dv.meta, (cudaStream_t)cuda_stream, &n);
   g_launches += n;
   return e == 0 ? LI_OK : LI_ERR_CUDA;
 }

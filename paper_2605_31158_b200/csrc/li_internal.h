@@ -40,6 +40,7 @@ struct SelectParams {
   int32_t *sel_cnt;
   float *scores;   // optional
   float inv_sqrt_d;
+  const float *slice_cache;   // 3-D tiling: per-page patch sums [n_pages,H,Hb*Wb,d]; non-null: kbar is formed from them
 };
 
 struct AttnParams {
@@ -66,7 +67,6 @@ constexpr int kMaxSplitSlots = 320;   // upper bound of split CTAs (<= 2 CTAs pe
 // launches (defined in the .cu files); return cudaError_t as int
 int launch_select(const SelectParams &sp, const BatchMeta &meta, cudaStream_t st, int64_t *n_launches);
 int launch_pool_pages(const SelectParams &sp, const int32_t *pages, int n_list, float *cache, cudaStream_t st, int64_t *n_launches);
-int launch_kbar_from_slices(const SelectParams &sp, const BatchMeta &meta, const float *cache, cudaStream_t st, int64_t *n_launches);
 int launch_attn(const AttnParams &ap, const BatchMeta &meta, int d, int blk, const CUtensorMap &tm_q,
                 const CUtensorMap &tm_tk, const CUtensorMap &tm_tv, const CUtensorMap &tm_k_full, const CUtensorMap &tm_k_8, const CUtensorMap &tm_v_full,
                 const CUtensorMap &tm_v_8, cudaStream_t st, int64_t *n_launches);

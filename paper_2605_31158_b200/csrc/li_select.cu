@@ -102,6 +102,18 @@ __global__ void __launch_bounds__(kPoolThreads) li_pool_kernel(const SelectParam
     uint4 v[kMaxIter];
     if constexpr (K3D) {
       nvalid = count3d(m, n_hist);
+      if (p.slice_cache != nullptr) {
+        // page-resident patch sums (li_pool_pages): the block mean from <= bt cached rows, one channel per thread
+        if (threadIdx.x < D) {
+          const int per = tl.Hb * tl.Wb, tg = m / per, patch = m - tg * per;
+          const int nf = min(tl.bt, n_hist - tg * tl.bt);
+          float s = 0.f;
+          for (int f = 0; f < nf; ++f)
+            s += __ldg(p.slice_cache + (((int64_t)__ldg(pages + tg * tl.bt + f) * p.H + h) * per + patch) * D + threadIdx.x);
+          p.kbar[(((int64_t)b * p.H + h) * D + threadIdx.x) * p.Mp + m] = s / (float)nvalid;
+        }
+        return;
+      }
 #pragma unroll
       for (int it = 0; it < kMaxIter; ++it) {
         const int r = r0 + it * RPP;
@@ -333,39 +345,11 @@ __global__ void __launch_bounds__(128) li_pool_pages_kernel(const SelectParams p
   }
 }
 
-// kbar of every historical block from the cached patch sums of its frames.  grid (Mmax, H, B), D threads = channels.
-template <int D>
-__global__ void __launch_bounds__(D) li_kbar_from_slices_kernel(const SelectParams p, const BatchMeta meta, const float *cache) {
-  const Tiling tl = p.tl;
-  const int m = blockIdx.x, h = blockIdx.y, b = blockIdx.z, c = threadIdx.x;
-  const int foff = meta.frame_off[b];
-  const int n_hist = meta.frame_off[b + 1] - foff - p.n_cur;
-  if (m >= tl.num_blocks(n_hist, p.T_f, p.blk)) return;
-  const int per = tl.Hb * tl.Wb, tg = m / per, patch = m - tg * per, hb = patch / tl.Wb;
-  const int nf = min(tl.bt, n_hist - tg * tl.bt);
-  float s = 0.f;
-  for (int f = 0; f < nf; ++f) {
-    const int page = __ldg(p.frame_idx + foff + tg * tl.bt + f);
-    s += __ldg(cache + (((int64_t)page * p.H + h) * per + patch) * D + c);
-  }
-  const int nvalid = nf * min(tl.bh, tl.gh - hb * tl.bh) * tl.bw;                    // Eq. 9: true cardinality |K_m|
-  p.kbar[(((int64_t)b * p.H + h) * D + c) * p.Mp + m] = s / (float)nvalid;         // kbar is [B,H,d,Mp]
-}
-
 int launch_pool_pages(const SelectParams &sp, const int32_t *pages, int n_list, float *cache, cudaStream_t st, int64_t *n_launches) {
   if (n_list <= 0) return 0;
   dim3 grid(sp.tl.Hb * sp.tl.Wb, sp.H, n_list);
   if (sp.d == 128) li_pool_pages_kernel<128><<<grid, 128, 0, st>>>(sp, pages, cache);
   else li_pool_pages_kernel<64><<<grid, 128, 0, st>>>(sp, pages, cache);
-  if (n_launches) *n_launches += 1;
-  return (int)cudaGetLastError();
-}
-
-int launch_kbar_from_slices(const SelectParams &sp, const BatchMeta &meta, const float *cache, cudaStream_t st, int64_t *n_launches) {
-  if (sp.Mmax <= 0) return 0;
-  dim3 grid(sp.Mmax, sp.H, sp.B);
-  if (sp.d == 128) li_kbar_from_slices_kernel<128><<<grid, 128, 0, st>>>(sp, meta, cache);
-  else li_kbar_from_slices_kernel<64><<<grid, 64, 0, st>>>(sp, meta, cache);
   if (n_launches) *n_launches += 1;
   return (int)cudaGetLastError();
 }
