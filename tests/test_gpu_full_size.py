@@ -84,3 +84,24 @@ def test_mid3d_full_size_mask_and_sampled_attention(P):
     mx, mean = P.compare_output(buf.o, buf.lse, o_ref, lse_ref, mask=mask)
     print(f"mid3d: {excused} excused rows, max-abs {mx:.3g}, mean-abs {mean:.3g}")
     assert torch.isfinite(buf.o.float()).all() and torch.isfinite(buf.lse).all()      # every token written, none NaN
+
+
+def test_long3d_full_size_mask_and_sampled_attention(P):
+    """`long` shapes (32 history frames, K offsets per page and head, density 1/10) with 3-D (4,8,4) blocks: 416 history
+    blocks, k = 41; 1248 query blocks = 4.22 waves, so the tail-wave split runs at full size."""
+    import paper_2605_31158_b200 as li
+    prob = W.build(W.spec_long3d())
+    assert prob.M(0) == 416 and prob.Nqb == 52 and int(prob.top_k[0]) == 41
+    li.lib().li_reset_launch_count()
+    ctx, buf = P.run_gpu(prob, want_scores=True)
+    assert li.lib().li_launch_count() == 5
+    osel, osc = P.oracle_select(prob)
+    excused = P.check_selection(prob, buf, osel, osc)
+    gsel = [g[0] for g in P.gpu_selection(prob, buf)]
+    tiles = [(0, 0, 0), (0, 23, 51), (0, 5, 40), (0, 17, 13)]          # 51 = last split query block, 40 = a 96-token border block
+    o_ref, lse_ref = P.oracle_attn(prob, gsel, tiles=tiles)
+    mask = ~np.isnan(lse_ref)
+    assert mask.sum() == 2 * 128 + 2 * 96
+    mx, mean = P.compare_output(buf.o, buf.lse, o_ref, lse_ref, mask=mask)
+    print(f"long3d: {excused} excused rows, max-abs {mx:.3g}, mean-abs {mean:.3g}")
+    assert torch.isfinite(buf.o.float()).all() and torch.isfinite(buf.lse).all()
