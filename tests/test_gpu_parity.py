@@ -329,3 +329,16 @@ def test_whole_step_is_cuda_graph_capturable(P):
         graph.replay()
         torch.cuda.synchronize()
         assert torch.equal(buf.sel_idx, sel) and torch.equal(buf.o, o) and torch.equal(buf.lse, lse)
+
+
+@pytest.mark.parametrize("d,block", [(64, 64), (128, 64), (64, 128)])
+def test_tail_wave_split_other_tile_shapes(P, d, block):
+    """The split instances of the other (d, block) template variants: 64-key blocks (32-key half-tiles) and d = 64."""
+    import paper_2605_31158_b200 as li
+    spec = W.spec_small(name=f"small-split-{d}-{block}", H=2, d=d, block=block, frame_tokens=72, n_cur_frames=3, n_pages=48,
+                        n_mem=(12,), n_win=(28,), density=Fraction(1, 1))
+    prob = W.build(spec)
+    li.lib().li_reset_launch_count()
+    excused, mx, mean = P.full_parity(prob)
+    assert li.lib().li_launch_count() == 5, "split not taken"
+    print(f"small-split d={d} block={block}: excused={excused} max-abs={mx:.3g} mean-abs={mean:.3g}")
