@@ -478,7 +478,7 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
           tc_fence_after();
           const float f = need ? ex2_approx(m_used - m_new) : 1.0f;
           if (need) { m_used = m_new; l *= f; }
-#pragma unroll
+#pragma unroll 1
           for (int c = 0; c < D / 32; ++c) {
             uint32_t o[32];
             tmem_ld32(tmem + lane_base + kOCol + c * 32, o);
