@@ -342,3 +342,22 @@ def test_tail_wave_split_other_tile_shapes(P, d, block):
     excused, mx, mean = P.full_parity(prob)
     assert li.lib().li_launch_count() == 5, "split not taken"
     print(f"small-split d={d} block={block}: excused={excused} max-abs={mx:.3g} mean-abs={mean:.3g}")
+
+
+def test_outputs_are_bitwise_repeatable(P):
+    """No atomics on data, fixed reduction orders, every hand-off through mbarriers: repeated runs (also with the
+    tail-wave split and its merge) must reproduce mask, O and LSE bit for bit -- a race would show up here."""
+    import paper_2605_31158_b200 as li
+    spec = W.spec_small(name="small-repeat", H=2, d=128, block=128, frame_tokens=200, n_cur_frames=3, n_pages=24,
+                        n_mem=(6,), n_win=(14,), density=Fraction(1, 2))
+    prob = W.build(spec)
+    ctx, buf = P.run_gpu(prob, want_scores=False)
+    ref = (buf.sel_idx.clone(), buf.o.clone(), buf.lse.clone())
+    junk = torch.empty(64 << 20, dtype=torch.uint8, device="cuda")
+    for it in range(20):
+        if it % 2:
+            junk.fill_(it)                                  # perturb cache state and timing
+        buf.sel_idx.fill_(-5); buf.o.fill_(float("nan")); buf.lse.fill_(float("nan"))
+        li.forward(ctx, prob.top_k, buf)
+        torch.cuda.synchronize()
+        assert torch.equal(buf.sel_idx, ref[0]) and torch.equal(buf.o, ref[1]) and torch.equal(buf.lse, ref[2]), it
