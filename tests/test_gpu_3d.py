@@ -169,3 +169,33 @@ def test_select_from_page_resident_patch_sums(P, grid, block3d, n_cur, n_hist, d
             M = prob.M(b)
             torch.testing.assert_close(sc_cached[b, :, :, :M], buf.scores[b, :, :, :M], rtol=1e-5, atol=1e-6)
     print(f"cached select {grid} {block3d}: excused={excused}")
+
+
+def test_text_prefix_3d_with_tail_wave_split(P):
+    """Text prefix + 3-D blocks + split query blocks in one launch (the TEXT x K3D x SPLIT kernel instance)."""
+    import paper_2605_31158_b200 as li
+    from oracle import li_oracle as O
+    spec = small3d("text-3d-split", (10, 16), (4, 8, 4), 4, (8,), (12,), density=Fraction(1, 1), n_pages=30)
+    prob = W.build(spec)
+    Lt = 200
+    g = torch.Generator().manual_seed(777)
+    tk = torch.randn((1, spec.H, Lt, spec.d), generator=g).to(torch.bfloat16)
+    tv = torch.randn((1, spec.H, Lt, spec.d), generator=g).to(torch.bfloat16)
+    ctx = li.Context(prob.q.cuda(), prob.k_cache.cuda(), prob.v_cache.cuda(), torch.from_numpy(prob.frame_idx).cuda(),
+                     prob.frame_off, spec.n_cur_frames, spec.block, grid=spec.grid, block3d=spec.block3d,
+                     text_k=tk.cuda(), text_v=tv.cuda())
+    buf = li.Buffers(ctx, prob.kmax, want_scores=True)
+    buf.o.fill_(float("nan"))
+    li.lib().li_reset_launch_count()
+    li.forward(ctx, prob.top_k, buf)
+    torch.cuda.synchronize()
+    assert li.lib().li_launch_count() == 5, "split not taken"
+    osel, osc = P.oracle_select(prob)
+    P.check_selection(prob, buf, osel, osc)
+    gsel = [g_[0] for g_ in P.gpu_selection(prob, buf)]
+    u16 = lambda t: t.contiguous().view(torch.int16).numpy().view(np.uint16)
+    s = spec
+    o_ref, lse_ref = O.sparse_attn_3d(prob.u16(prob.q), prob.u16(prob.k_cache), prob.u16(prob.v_cache), prob.frame_idx,
+                                      prob.frame_off, s.n_cur_frames, *s.grid, *s.block3d, gsel, text_k=u16(tk), text_v=u16(tv))
+    mx, mean = P.compare_output(buf.o, buf.lse, o_ref, lse_ref)
+    print(f"text-3d-split: max-abs {mx:.3g} mean-abs {mean:.3g}")
