@@ -34,6 +34,7 @@ UNIT = "TFLOP/s"
 # dram__bytes_read.sum + dram__bytes_write.sum of li_sparse_attn_kernel<128,128> per launch, from the
 # `ncu --set full` capture summarised in profiles/ (None until that capture exists for this workload).
 NCU_TRAFFIC_BYTES = {"mid": 400871936,     # profiles/r1d_mid_ncu_full_summary.txt: 366.19 MB read + 34.68 MB written
+                     "long": 1082519360,   # gpurun capture r1d (ncu --set full, same command with --config long): 1048.78 MB + 33.74 MB
                      "mid3d": 408045056}   # profiles/r1b_mid3d_attn_ncu_summary.txt: 375.72 MB + 32.33 MB (split kernel)
 
 
