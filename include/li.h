@@ -12,7 +12,9 @@
  *
  * Conventions
  *   - Every pointer is a DEVICE pointer unless its name ends in _host.  The caller owns every buffer; the
- *     library never allocates or frees device memory and keeps no global state besides loaded kernels.
+ *     library never allocates or frees device memory.  Process-wide state: the loaded kernels, a small cache of
+ *     encoded TMA descriptors (keyed by address, shape and strides, so a steady-state call does no driver work), the
+ *     launch counter, and a thread-local copy of the last CUDA error code.  No environment variable is read.
  *   - Calls are asynchronous on `cuda_stream` (a cudaStream_t passed as void*; NULL = default stream) and
  *     never synchronise the device.  Host arrays are consumed before the call returns.
  *   - Return value: LI_OK (0) or a negative LI_ERR_* code.  No C++ exception crosses this boundary.
@@ -36,7 +38,7 @@
 extern "C" {
 #endif
 
-#define LI_VERSION 102          /* major*100 + minor */
+#define LI_VERSION 200          /* major*100 + minor */
 #define LI_MAX_CALLS 64         /* max B per call of the library (batch of independent attention calls) */
 
 enum {
@@ -44,8 +46,12 @@ enum {
   LI_ERR_INVALID_ARG = -1,      /* NULL pointer, non-positive size, bad stride/alignment, bad frame list */
   LI_ERR_UNSUPPORTED = -2,      /* d not in {64,128}; block not in {64,128}; block_q != block_k; B > LI_MAX_CALLS */
   LI_ERR_WORKSPACE   = -3,      /* workspace NULL or smaller than li_workspace_bytes() */
-  LI_ERR_CUDA        = -4       /* a CUDA runtime/driver call failed (no device, launch error, ...) */
+  LI_ERR_CUDA        = -4       /* a CUDA runtime/driver call failed (no device, launch error, ...); the runtime's own
+                                   code is returned by li_last_cuda_error() */
 };
+
+/* li_problem.flags */
+#define LI_FLAG_NO_SPLIT 1u     /* li_sparse_attn: never split the query blocks of the last wave */
 
 typedef struct li_problem {
   int32_t B, H, Lq, d;          /* B independent calls; Lq = n_cur_frames * frame_tokens when n_cur_frames > 0 */
@@ -78,6 +84,7 @@ typedef struct li_problem {
   const void *text_k;           /* bf16 [B,H,Lt,d] */
   const void *text_v;           /* bf16, same shape and strides */
   int64_t t_sb, t_sh, t_st;     /* batch / head / token strides of both */
+  uint32_t flags;               /* LI_FLAG_* bits, 0 = defaults */
 } li_problem;
 
 /* Eq. 9-10.  For every call b, head h and query block i: pooled means (true cardinality
@@ -124,13 +131,32 @@ int li_block_select_cached(const li_problem *p, const int32_t *top_k_host, int32
  *   o       : bf16 [B,H,Lq,d], contiguous.
  *   lse_opt : NULL or fp32 [B,H,Lq]: log sum_n exp(scale * q.k_n) (natural log).
  * An empty context (no chunk and no selected block) gives o = 0, lse = -inf.
- * sel_idx values must lie in [0, M_b); they are not validated on the host.
+ * sel_idx rows are SETS: the first sel_cnt entries of a row must be distinct values in [0, M_b), in ANY order (the
+ * blocks are attended in the order given; li_block_select writes them ascending); sel_cnt <= kmax.  Neither is checked
+ * by this call (device data): li_validate checks them on the device.
  *   workspace : optional.  With >= li_workspace_bytes(p, kmax) bytes (256-byte aligned; the same buffer li_block_select
  *               used: its pooled keys are left intact) the kernel may split the query blocks of a sparsely filled last
  *               wave of CTAs across several CTAs and merge their partial results with a second, small launch
  *               (results equal up to fp32 rounding of the merge).  NULL or a smaller buffer: never split. */
 int li_sparse_attn(const li_problem *p, const int32_t *sel_idx, const int32_t *sel_cnt, int32_t kmax,
                    void *o, float *lse_opt, void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* Debug validation of DEVICE-side inputs that the calls above trust (one small launch, asynchronous, no host
+ * synchronisation; meant for debug builds of the caller, not for the hot loop):
+ *   - every page id of every call's frame list lies in [0, n_pages)                                   LI_BAD_PAGE_ID
+ *   - when sel_idx/sel_cnt are given (both or neither): 0 <= sel_cnt <= min(kmax, M_b)                LI_BAD_SEL_CNT
+ *     every one of the first sel_cnt entries lies in [0, M_b)                                         LI_BAD_SEL_RANGE
+ *     and the entries of a row are distinct (checked for M_b <= 262144)                               LI_BAD_SEL_DUPLICATE
+ * error_dev: DEVICE int32[4], overwritten: [0] = OR of the LI_BAD_* bits found (0 = all good), [1] = call b,
+ * [2] = position (frame-list entry, or flat (h*Nqb + i)*kmax + t) and [3] = value of ONE offender (the lowest bit's
+ * first-arriving report; which one is unspecified when several exist).  Without it a bad page id is an out-of-bounds
+ * read in li_block_select and a silently zero-filled tile in li_sparse_attn. */
+#define LI_BAD_PAGE_ID 1
+#define LI_BAD_SEL_CNT 2
+#define LI_BAD_SEL_RANGE 4
+#define LI_BAD_SEL_DUPLICATE 8
+int li_validate(const li_problem *p, const int32_t *sel_idx, const int32_t *sel_cnt, int32_t kmax,
+                int32_t *error_dev, void *cuda_stream);
 
 /* Bytes of workspace the calls above need for problem p (0 on invalid p): li_block_select's pooled means and score keys,
  * followed by the partial-result buffers of li_sparse_attn's split (a fixed ~21 MB at d = 128). */
@@ -188,6 +214,8 @@ void li_reset_launch_count(void);
 
 const char *li_strerror(int code);
 int li_version(void);
+/* cudaError_t of the last call of THIS thread that returned LI_ERR_CUDA (0 if none). */
+int li_last_cuda_error(void);
 
 #ifdef __cplusplus
 }

@@ -18,16 +18,20 @@ LIB_PATH = os.path.join(_HERE, "libli.so")
 
 LI_OK, LI_ERR_INVALID_ARG, LI_ERR_UNSUPPORTED, LI_ERR_WORKSPACE, LI_ERR_CUDA = 0, -1, -2, -3, -4
 LI_MAX_CALLS = 64
+LI_FLAG_NO_SPLIT = 1
+LI_BAD_PAGE_ID, LI_BAD_SEL_CNT, LI_BAD_SEL_RANGE, LI_BAD_SEL_DUPLICATE = 1, 2, 4, 8
 
 EXPORTS = ("li_block_select", "li_block_select_reuse_kbar", "li_block_select_cached", "li_pool_pages", "li_slice_cache_bytes",
-           "li_sparse_attn", "li_workspace_bytes", "li_context_policy",
-           "li_policy_workspace_bytes", "li_launch_count", "li_reset_launch_count", "li_strerror", "li_version")
+           "li_sparse_attn", "li_validate", "li_workspace_bytes", "li_context_policy",
+           "li_policy_workspace_bytes", "li_launch_count", "li_reset_launch_count", "li_strerror", "li_version",
+           "li_last_cuda_error")
 
 
 class LiError(RuntimeError):
     def __init__(self, code: int, where: str):
         self.code = code
-        super().__init__(f"{where}: {strerror(code)} ({code})")
+        extra = f", cudaError {lib().li_last_cuda_error()}" if code == LI_ERR_CUDA else ""
+        super().__init__(f"{where}: {strerror(code)} ({code}{extra})")
 
 
 class li_problem(ctypes.Structure):
@@ -45,6 +49,7 @@ class li_problem(ctypes.Structure):
         ("bt", ctypes.c_int32), ("bh", ctypes.c_int32), ("bw", ctypes.c_int32),
         ("Lt", ctypes.c_int32), ("text_k", ctypes.c_void_p), ("text_v", ctypes.c_void_p),
         ("t_sb", ctypes.c_int64), ("t_sh", ctypes.c_int64), ("t_st", ctypes.c_int64),
+        ("flags", ctypes.c_uint32),
     ]
 
 
@@ -103,6 +108,10 @@ def lib() -> ctypes.CDLL:
         L.li_context_policy.restype = ctypes.c_int
         L.li_context_policy.argtypes = [ctypes.POINTER(li_policy), ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p,
                                         ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p]
+        L.li_validate.restype = ctypes.c_int
+        L.li_validate.argtypes = [P, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p, ctypes.c_void_p]
+        L.li_last_cuda_error.restype = ctypes.c_int
+        L.li_last_cuda_error.argtypes = []
         L.li_launch_count.restype = ctypes.c_int64
         L.li_reset_launch_count.restype = None
         L.li_strerror.restype = ctypes.c_char_p
@@ -134,7 +143,7 @@ class Context:
     def __init__(self, q: torch.Tensor, k_cache: torch.Tensor, v_cache: torch.Tensor, frame_idx: torch.Tensor,
                  frame_off: Sequence[int], n_cur_frames: int, block: int, softmax_scale: float = 0.0,
                  grid: Optional[Tuple[int, int]] = None, block3d: Optional[Tuple[int, int, int]] = None,
-                 text_k: Optional[torch.Tensor] = None, text_v: Optional[torch.Tensor] = None):
+                 text_k: Optional[torch.Tensor] = None, text_v: Optional[torch.Tensor] = None, flags: int = 0):
         for t, name in ((q, "q"), (k_cache, "k_cache"), (v_cache, "v_cache")):
             if t.dtype != torch.bfloat16 or not t.is_cuda or t.dim() != 4 or t.stride(-1) != 1:
                 raise ValueError(f"{name} must be a 4-D CUDA bf16 tensor with unit innermost stride")
@@ -160,6 +169,7 @@ class Context:
         p.frame_off_host = self.frame_off.ctypes.data
         p.n_cur_frames = n_cur_frames
         p.softmax_scale = softmax_scale
+        p.flags = int(flags)
         self.text_k, self.text_v = text_k, text_v
         if text_k is not None:
             for t, name in ((text_k, "text_k"), (text_v, "text_v")):
@@ -261,6 +271,19 @@ def li_sparse_attn(ctx: Context, sel_idx: torch.Tensor, sel_cnt: torch.Tensor, k
                               _stream_ptr(stream))
     if rc != LI_OK:
         raise LiError(rc, "li_sparse_attn")
+
+
+def li_validate(ctx: Context, error: torch.Tensor, sel_idx: Optional[torch.Tensor] = None,
+                sel_cnt: Optional[torch.Tensor] = None, kmax: int = 0, stream: Optional[torch.cuda.Stream] = None) -> None:
+    """li_validate (include/li.h): device-side check of the frame lists (and of sel_idx / sel_cnt when given) into
+    `error`, an int32 CUDA tensor of 4 entries: [LI_BAD_* bits, 1 + call, position, value]."""
+    if error.dtype != torch.int32 or not error.is_cuda or error.numel() < 4 or not error.is_contiguous():
+        raise ValueError("error must be a contiguous int32 CUDA tensor of >= 4 entries")
+    rc = lib().li_validate(ctypes.byref(ctx.p), sel_idx.data_ptr() if sel_idx is not None else None,
+                           sel_cnt.data_ptr() if sel_cnt is not None else None, int(kmax), error.data_ptr(),
+                           _stream_ptr(stream))
+    if rc != LI_OK:
+        raise LiError(rc, "li_validate")
 
 
 class Buffers:

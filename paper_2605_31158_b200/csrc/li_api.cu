@@ -1,17 +1,23 @@
 // li_api.cu -- the C ABI of libli.so (include/li.h): argument validation, workspace carving, TMA tensor-map
-// encoding and kernel launches.  No device allocation, no synchronisation, no global state except the
-// launch counter and the lazily resolved cuTensorMapEncodeTiled entry point.
+// encoding and kernel launches.  No device allocation, no synchronisation, no environment variable.  Process-wide
+// state: the launch counter, the lazily resolved cuTensorMapEncodeTiled entry point, a small cache of encoded tensor
+// maps (a steady-state call does no driver work) and a thread-local copy of the last CUDA error code.
 #include <atomic>
 #include <cmath>
-#include <cstdio>
-#include <cstdlib>
 #include <cstring>
+#include <mutex>
 
 #include "li_internal.h"
 
 namespace {
 
 std::atomic<int64_t> g_launches{0};
+thread_local int t_last_cuda_error = 0;
+
+int cuda_failed(int e) {
+  t_last_cuda_error = e;
+  return LI_ERR_CUDA;
+}
 
 using EncodeFn = CUresult (*)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                               const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
@@ -30,36 +36,74 @@ EncodeFn get_encode() {
   return reinterpret_cast<EncodeFn>(fn);
 }
 
+// Encoded tensor maps are pure functions of (address, shape, strides, box): they are cached, so that a call with the
+// same tensors as an earlier one (the steady state of an AR loop) does no driver work.
+struct MapKey {
+  const void *base;
+  int32_t rank, d, box[4];
+  int64_t dims[4], strides[4];
+  bool operator==(const MapKey &o) const { return std::memcmp(this, &o, sizeof(MapKey)) == 0; }
+};
+struct MapCache {
+  static constexpr int kEntries = 64;
+  std::mutex mu;
+  MapKey keys[kEntries];
+  CUtensorMap maps[kEntries];
+  int used = 0, next = 0;
+};
+MapCache g_maps;
+
+bool encode_cached(CUtensorMap *tm, const MapKey &key) {
+  {
+    std::lock_guard<std::mutex> lock(g_maps.mu);
+    for (int e = 0; e < g_maps.used; ++e)
+      if (g_maps.keys[e] == key) { *tm = g_maps.maps[e]; return true; }
+  }
+  EncodeFn enc = get_encode();
+  if (enc == nullptr) return false;
+  cuuint64_t dims[5] = {(cuuint64_t)key.d};
+  cuuint64_t strides[4];
+  cuuint32_t box[5] = {64}, estr[5] = {1, 1, 1, 1, 1};
+  for (int k = 0; k + 1 < key.rank; ++k) {
+    dims[k + 1] = (cuuint64_t)key.dims[k];
+    strides[k] = (cuuint64_t)key.strides[k] * 2;
+    box[k + 1] = (cuuint32_t)key.box[k];
+  }
+  CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, (cuuint32_t)key.rank, const_cast<void *>(key.base), dims, strides, box,
+                   estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return false;
+  std::lock_guard<std::mutex> lock(g_maps.mu);
+  const int slot = g_maps.used < MapCache::kEntries ? g_maps.used++ : (g_maps.next++ % MapCache::kEntries);
+  g_maps.keys[slot] = key;
+  g_maps.maps[slot] = *tm;
+  return true;
+}
+
 // bf16 tensor [n3, n2, n1, d] (innermost first: d, n1, n2, n3), strides in elements, box = 64 x rows x 1 x 1,
 // SWIZZLE_128B, out-of-bounds elements read as zero.
 bool encode_map(CUtensorMap *tm, const void *base, int d, int64_t n1, int64_t n2, int64_t n3, int64_t s1, int64_t s2,
                 int64_t s3, int box_rows) {
-  EncodeFn enc = get_encode();
-  if (enc == nullptr) return false;
-  cuuint64_t dims[4] = {(cuuint64_t)d, (cuuint64_t)n1, (cuuint64_t)n2, (cuuint64_t)n3};
-  cuuint64_t strides[3] = {(cuuint64_t)s1 * 2, (cuuint64_t)s2 * 2, (cuuint64_t)s3 * 2};
-  cuuint32_t box[4] = {64, (cuuint32_t)box_rows, 1, 1};
-  cuuint32_t estr[4] = {1, 1, 1, 1};
-  CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void *>(base), dims, strides, box, estr,
-                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  return r == CUDA_SUCCESS;
+  MapKey k;
+  std::memset(&k, 0, sizeof(k));
+  k.base = base; k.rank = 4; k.d = d;
+  k.dims[0] = n1; k.dims[1] = n2; k.dims[2] = n3;
+  k.strides[0] = s1; k.strides[1] = s2; k.strides[2] = s3;
+  k.box[0] = box_rows; k.box[1] = 1; k.box[2] = 1;
+  return encode_cached(tm, k);
 }
 
 // bf16 tensor viewed as 5-D [n4, n3, gh, gw, d] (innermost first: d, gw, gh, n3, n4), box = 64 x bw x bh x 1 x 1:
 // one frame's bh x bw patch of a 3-D block = 32 rows of 128 bytes, SWIZZLE_128B, zero fill outside.
 bool encode_map5(CUtensorMap *tm, const void *base, int d, int gw, int gh, int64_t n3, int64_t n4, int64_t s_w,
                  int64_t s_h, int64_t s3, int64_t s4, int bw, int bh) {
-  EncodeFn enc = get_encode();
-  if (enc == nullptr) return false;
-  cuuint64_t dims[5] = {(cuuint64_t)d, (cuuint64_t)gw, (cuuint64_t)gh, (cuuint64_t)n3, (cuuint64_t)n4};
-  cuuint64_t strides[4] = {(cuuint64_t)s_w * 2, (cuuint64_t)s_h * 2, (cuuint64_t)s3 * 2, (cuuint64_t)s4 * 2};
-  cuuint32_t box[5] = {64, (cuuint32_t)bw, (cuuint32_t)bh, 1, 1};
-  cuuint32_t estr[5] = {1, 1, 1, 1, 1};
-  CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 5, const_cast<void *>(base), dims, strides, box, estr,
-                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  return r == CUDA_SUCCESS;
+  MapKey k;
+  std::memset(&k, 0, sizeof(k));
+  k.base = base; k.rank = 5; k.d = d;
+  k.dims[0] = gw; k.dims[1] = gh; k.dims[2] = n3; k.dims[3] = n4;
+  k.strides[0] = s_w; k.strides[1] = s_h; k.strides[2] = s3; k.strides[3] = s4;
+  k.box[0] = bw; k.box[1] = bh; k.box[2] = 1; k.box[3] = 1;
+  return encode_cached(tm, k);
 }
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -71,9 +115,30 @@ struct Derived {
   li::BatchMeta meta;
 };
 
-// Validates p and fills the derived integers.  Returns LI_OK or an error code.
-int check_problem(const li_problem *p, Derived *dv) {
+// Validates p and fills the derived integers.  Returns LI_OK or an error code.  pages_only: the call touches only the
+// K cache and the tiling (li_pool_pages, li_slice_cache_bytes): Q, the frame lists and the text region are not looked at.
+int check_problem(const li_problem *p, Derived *dv, bool pages_only = false) {
   if (p == nullptr) return LI_ERR_INVALID_ARG;
+  if (pages_only) {
+    if (p->H <= 0 || p->frame_tokens <= 0 || p->n_pages <= 0) return LI_ERR_INVALID_ARG;
+    if (p->d != 64 && p->d != 128) return LI_ERR_UNSUPPORTED;
+    if (p->block_k != 64 && p->block_k != 128) return LI_ERR_UNSUPPORTED;
+    if (p->frame_tokens % 8 != 0 || p->k_cache == nullptr || ((uintptr_t)p->k_cache & 15u)) return LI_ERR_INVALID_ARG;
+    const int64_t ks[3] = {p->kv_sp, p->kv_sh, p->kv_st};
+    for (int64_t s : ks)
+      if (s <= 0 || s % 8 != 0) return LI_ERR_INVALID_ARG;
+    if (p->kv_st < p->d) return LI_ERR_INVALID_ARG;
+    std::memset(&dv->meta, 0, sizeof(dv->meta));
+    std::memset(&dv->tl, 0, sizeof(dv->tl));
+    if (p->grid_h <= 0 || p->grid_w <= 0 || p->bt <= 0 || p->bh <= 0 || p->bw <= 0) return LI_ERR_UNSUPPORTED;
+    if (p->grid_h * p->grid_w != p->frame_tokens) return LI_ERR_INVALID_ARG;
+    if (p->bt * p->bh * p->bw != p->block_k || p->bh * p->bw != 32 || p->grid_w % p->bw != 0) return LI_ERR_UNSUPPORTED;
+    dv->tl.gh = p->grid_h; dv->tl.gw = p->grid_w; dv->tl.bt = p->bt; dv->tl.bh = p->bh; dv->tl.bw = p->bw;
+    dv->tl.Hb = (p->grid_h + p->bh - 1) / p->bh; dv->tl.Wb = (p->grid_w + p->bw - 1) / p->bw;
+    for (dv->tl.bw_log2 = 0; (1 << dv->tl.bw_log2) < p->bw; ++dv->tl.bw_log2) {}
+    dv->Nqb = dv->Nc = dv->Mmax = 0;
+    return LI_OK;
+  }
   if (p->B <= 0 || p->H <= 0 || p->Lq <= 0 || p->frame_tokens <= 0 || p->n_pages <= 0 || p->n_cur_frames < 0)
     return LI_ERR_INVALID_ARG;
   if (p->d != 64 && p->d != 128) return LI_ERR_UNSUPPORTED;
@@ -109,7 +174,8 @@ int check_problem(const li_problem *p, Derived *dv) {
     if (p->bt * p->bh * p->bw != p->block_k || p->bh * p->bw != 32 || p->grid_w % p->bw != 0) return LI_ERR_UNSUPPORTED;
     if (p->q_sb != (int64_t)p->H * p->q_sh && p->B > 1) return LI_ERR_UNSUPPORTED;
     dv->tl.gh = p->grid_h; dv->tl.gw = p->grid_w; dv->tl.bt = p->bt; dv->tl.bh = p->bh; dv->tl.bw = p->bw;
-    dv->tl.Hb = (p->grid_h + p->bh - 1) / p->bh; dv->tl.Wb = p->grid_w / p->bw;
+    dv->tl.Hb = (p->grid_h + p->bh - 1) / p->bh; dv->tl.Wb = (p->grid_w + p->bw - 1) / p->bw;
+    for (dv->tl.bw_log2 = 0; (1 << dv->tl.bw_log2) < p->bw; ++dv->tl.bw_log2) {}
   }
   int mmax = 0;
   if (p->frame_off_host[0] < 0) return LI_ERR_INVALID_ARG;
@@ -176,7 +242,7 @@ static int block_select_impl(const li_problem *p, const int32_t *top_k_host, int
   sp.tl = dv.tl;
   sp.skip_k = skip_k;
   sp.B = p->B; sp.H = p->H; sp.Lq = p->Lq; sp.d = p->d; sp.T_f = p->frame_tokens; sp.blk = p->block_k;
-  sp.n_cur = p->n_cur_frames; sp.Nqb = dv.Nqb; sp.Mmax = dv.Mmax; sp.kmax = kmax;
+  sp.n_cur = p->n_cur_frames; sp.Nqb = dv.Nqb; sp.Mmax = dv.Mmax; sp.kmax = kmax; sp.n_pages = p->n_pages;
   sp.score_pitch = score_pitch;
   sp.q = (const uint16_t *)p->q; sp.q_sb = p->q_sb; sp.q_sh = p->q_sh; sp.q_st = p->q_st;
   sp.k_cache = (const uint16_t *)p->k_cache; sp.kv_sp = p->kv_sp; sp.kv_sh = p->kv_sh; sp.kv_st = p->kv_st;
@@ -192,31 +258,30 @@ static int block_select_impl(const li_problem *p, const int32_t *top_k_host, int
   sp.slice_cache = slice_cache;             // non-null: the pool kernel forms kbar from the cached patch sums
   e = li::launch_select(sp, dv.meta, (cudaStream_t)cuda_stream, &n);
   g_launches += n;
-  return e == 0 ? LI_OK : LI_ERR_CUDA;
+  return e == 0 ? LI_OK : cuda_failed(e);
 }
 
 size_t li_slice_cache_bytes(const li_problem *p) {
   Derived dv;
-  if (check_problem(p, &dv) != LI_OK || dv.tl.bt == 0) return 0;
+  if (check_problem(p, &dv, true) != LI_OK) return 0;
   return (size_t)p->n_pages * p->H * dv.tl.Hb * dv.tl.Wb * p->d * 4;
 }
 
 int li_pool_pages(const li_problem *p, const int32_t *pages_dev, int32_t n_list, float *slice_cache, void *cuda_stream) {
   Derived dv;
-  int rc = check_problem(p, &dv);
+  int rc = check_problem(p, &dv, true);
   if (rc != LI_OK) return rc;
-  if (dv.tl.bt == 0) return LI_ERR_UNSUPPORTED;
   if (n_list < 0 || slice_cache == nullptr || (n_list > 0 && pages_dev == nullptr) || ((uintptr_t)slice_cache & 15u))
     return LI_ERR_INVALID_ARG;
   li::SelectParams sp;
   std::memset(&sp, 0, sizeof(sp));
   sp.tl = dv.tl;
-  sp.H = p->H; sp.d = p->d;
+  sp.H = p->H; sp.d = p->d; sp.n_pages = p->n_pages;
   sp.k_cache = (const uint16_t *)p->k_cache; sp.kv_sp = p->kv_sp; sp.kv_sh = p->kv_sh; sp.kv_st = p->kv_st;
   int64_t n = 0;
   const int e = li::launch_pool_pages(sp, pages_dev, n_list, slice_cache, (cudaStream_t)cuda_stream, &n);
   g_launches += n;
-  return e == 0 ? LI_OK : LI_ERR_CUDA;
+  return e == 0 ? LI_OK : cuda_failed(e);
 }
 
 int li_block_select_cached(const li_problem *p, const int32_t *top_k_host, int32_t kmax, int32_t *sel_idx,
@@ -283,13 +348,14 @@ int li_sparse_attn(const li_problem *p, const int32_t *sel_idx, const int32_t *s
     ok = ok && encode_map(&tm_tk, p->text_k, p->d, p->Lt, p->H, p->B, p->t_st, p->t_sh, p->t_sb, half);
     ok = ok && encode_map(&tm_tv, p->text_v, p->d, p->Lt, p->H, p->B, p->t_st, p->t_sh, p->t_sb, half);
   }
-  if (!ok) return LI_ERR_CUDA;
+  if (!ok) return cuda_failed((int)cudaErrorUnknown);
 
   li::AttnParams ap;
   std::memset(&ap, 0, sizeof(ap));
   ap.tl = dv.tl;
   ap.B = p->B; ap.H = p->H; ap.Lq = p->Lq; ap.T_f = p->frame_tokens; ap.n_cur = p->n_cur_frames;
   ap.Nqb = dv.Nqb; ap.Nc = dv.Nc; ap.kmax = kmax; ap.has_box_full = has_full; ap.Lt = p->Lt;
+  ap.no_split = (p->flags & LI_FLAG_NO_SPLIT) ? 1 : 0;
   const float scale = p->softmax_scale != 0.f ? p->softmax_scale : 1.0f / std::sqrt((float)p->d);
   ap.scale_log2 = scale * 1.4426950408889634f;
   ap.frame_idx = p->frame_idx; ap.sel_idx = sel_idx; ap.sel_cnt = sel_cnt;
@@ -301,9 +367,26 @@ int li_sparse_attn(const li_problem *p, const int32_t *sel_idx, const int32_t *s
   int64_t n = 0;
   const int e = li::launch_attn(ap, dv.meta, p->d, blk, tm_q, tm_tk, tm_tv, tm_kf, tm_k8, tm_vf, tm_v8, (cudaStream_t)cuda_stream, &n);
   g_launches += n;
-  if (e != 0 && std::getenv("LI_DEBUG") != nullptr)
-    std::fprintf(stderr, "li_sparse_attn: CUDA error %d: %s\n", e, cudaGetErrorString((cudaError_t)e));
-  return e == 0 ? LI_OK : LI_ERR_CUDA;
+  return e == 0 ? LI_OK : cuda_failed(e);
+}
+
+int li_validate(const li_problem *p, const int32_t *sel_idx, const int32_t *sel_cnt, int32_t kmax, int32_t *error_dev,
+                void *cuda_stream) {
+  Derived dv;
+  int rc = check_problem(p, &dv);
+  if (rc != LI_OK) return rc;
+  if (error_dev == nullptr || ((sel_idx == nullptr) != (sel_cnt == nullptr)) || (sel_idx != nullptr && kmax < 1))
+    return LI_ERR_INVALID_ARG;
+  li::ValidateParams vp;
+  std::memset(&vp, 0, sizeof(vp));
+  vp.tl = dv.tl;
+  vp.B = p->B; vp.H = p->H; vp.Nqb = dv.Nqb; vp.T_f = p->frame_tokens; vp.blk = p->block_k; vp.n_cur = p->n_cur_frames;
+  vp.n_pages = p->n_pages; vp.kmax = kmax; vp.Mmax = dv.Mmax;
+  vp.frame_idx = p->frame_idx; vp.sel_idx = sel_idx; vp.sel_cnt = sel_cnt; vp.err = error_dev;
+  int64_t n = 0;
+  const int e = li::launch_validate(vp, dv.meta, (cudaStream_t)cuda_stream, &n);
+  g_launches += n;
+  return e == 0 ? LI_OK : cuda_failed(e);
 }
 
 size_t li_policy_workspace_bytes(void) { return li::kPolicyWorkspaceBytes; }
@@ -326,7 +409,7 @@ int li_context_policy(const li_policy *pp, int32_t *frame_idx_out, int32_t frame
   int64_t n = 0;
   const int e = li::launch_policy(*pp, frame_idx_out, result_dev, (double *)workspace, (cudaStream_t)cuda_stream, &n);
   g_launches += n;
-  return e == 0 ? LI_OK : LI_ERR_CUDA;
+  return e == 0 ? LI_OK : cuda_failed(e);
 }
 
 int64_t li_launch_count(void) { return g_launches.load(); }
@@ -344,5 +427,6 @@ const char *li_strerror(int code) {
 }
 
 int li_version(void) { return LI_VERSION; }
+int li_last_cuda_error(void) { return t_last_cuda_error; }
 
 }  // extern "C"

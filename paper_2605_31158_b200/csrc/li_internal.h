@@ -19,6 +19,7 @@ struct BatchMeta {
 // m = (tg*Hb + hb)*Wb + wb; a block's rows are ordered (frame, y, x), 32 = bh*bw rows per frame slice.
 struct Tiling {
   int32_t gh, gw, bt, bh, bw, Hb, Wb;
+  int32_t bw_log2;                       // bh * bw == 32, so bw is a power of two
   __host__ __device__ int num_blocks(int n_frames, int T_f, int blk) const {
     return bt > 0 ? ((n_frames + bt - 1) / bt) * Hb * Wb : (n_frames * T_f + blk - 1) / blk;
   }
@@ -28,6 +29,7 @@ struct SelectParams {
   Tiling tl;
   int32_t skip_k;   // 1: kbar in the workspace is still valid (li_block_select_reuse_kbar): pool Q only
   int32_t B, H, Lq, d, T_f, blk, n_cur, Nqb, Mmax, Mp, kmax, score_pitch;   // Mp = Mmax rounded up to 32
+  int32_t n_pages;  // page ids outside [0, n_pages) are never dereferenced (their rows count as zeros; li_validate reports them)
   const uint16_t *q;
   int64_t q_sb, q_sh, q_st;
   const uint16_t *k_cache;
@@ -47,7 +49,8 @@ struct AttnParams {
   Tiling tl;
   int32_t B, H, Lq, T_f, n_cur, Nqb, Nc, kmax;
   int32_t Lt;             // text tokens (T of Eq. 11), 0 = none
-  int32_t has_box_full;   // 1: tensor maps with a full-block box exist (T_f >= block)
+  int32_t has_box_full;   // 1: tensor maps with a full half-tile box exist (T_f >= block/2)
+  int32_t no_split;       // LI_FLAG_NO_SPLIT
   float scale_log2;       // softmax_scale * log2(e)
   const int32_t *frame_idx;
   const int32_t *sel_idx;
@@ -70,6 +73,17 @@ int launch_pool_pages(const SelectParams &sp, const int32_t *pages, int n_list, 
 int launch_attn(const AttnParams &ap, const BatchMeta &meta, int d, int blk, const CUtensorMap &tm_q,
                 const CUtensorMap &tm_tk, const CUtensorMap &tm_tv, const CUtensorMap &tm_k_full, const CUtensorMap &tm_k_8, const CUtensorMap &tm_v_full,
                 const CUtensorMap &tm_v_8, cudaStream_t st, int64_t *n_launches);
+
+// li_validate (debug check of device-side inputs, include/li.h)
+struct ValidateParams {
+  Tiling tl;
+  int32_t B, H, Nqb, T_f, blk, n_cur, n_pages, kmax, Mmax;
+  const int32_t *frame_idx;
+  const int32_t *sel_idx;   // may be null (frame lists only)
+  const int32_t *sel_cnt;
+  int32_t *err;             // int32[4], zeroed before the launch
+};
+int launch_validate(const ValidateParams &vp, const BatchMeta &meta, cudaStream_t st, int64_t *n_launches);
 
 int launch_policy(const li_policy &pp, int32_t *frame_idx_out, li_policy_result *result, double *partial, cudaStream_t st,
                   int64_t *n_launches);

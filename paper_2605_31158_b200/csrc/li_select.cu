@@ -1,11 +1,15 @@
 // li_select.cu -- li_block_select for sm_100a (Eq. 9-10).
-//   kernel 1  li_pool_kernel       : block means of Q and of the historical K (K rows fetched through the
-//                                    frame-index list, in place).  HBM-bound streaming reduction: every Q and
-//                                    historical-K byte is read exactly once with 16-byte loads.
-//   kernel 2  li_score_kernel      : scores qbar_i . kbar_m / sqrt(d) (fp32) -> order-preserving uint32 keys.
-//   kernel 3  li_topk_kernel       : per-row top-k by an MSB-first radix select on the keys; ties -> lowest block
-//                                    index; indices written ascending.
+//   kernel 1  li_pool_kernel        : block means of Q and of the historical K (K rows fetched through the
+//                                     frame-index list, in place).  HBM-bound streaming reduction: every Q and
+//                                     historical-K byte is read exactly once with 16-byte loads.
+//   kernel 2  li_score_topk_kernel  : one warp per (call, head, query block) row: scores qbar_i . kbar_m / sqrt(d)
+//                                     (fp32) stay in registers as order-preserving keys, an MSB-first radix select
+//                                     finds the k-th largest, ties -> lowest block index, indices written ascending.
+//   (M > 512 historical blocks: li_score_kernel writes the keys to the workspace and li_topk_kernel selects from there.)
+#include <atomic>
+
 #include "li_internal.h"
+#include "li_ptx.cuh"
 
 namespace li {
 
@@ -21,157 +25,271 @@ __device__ __forceinline__ uint4 ldg_stream(const void *p) {
                : "l"(p));
   return r;
 }
-__device__ __forceinline__ void add_bf16x8(float (&acc)[8], const uint4 &v) {
-  acc[0] += __uint_as_float(v.x << 16);
-  acc[1] += __uint_as_float(v.x & 0xffff0000u);
-  acc[2] += __uint_as_float(v.y << 16);
-  acc[3] += __uint_as_float(v.y & 0xffff0000u);
-  acc[4] += __uint_as_float(v.z << 16);
-  acc[5] += __uint_as_float(v.z & 0xffff0000u);
-  acc[6] += __uint_as_float(v.w << 16);
-  acc[7] += __uint_as_float(v.w & 0xffff0000u);
+// 8 bf16 -> four packed fp32 pairs, accumulated with add.rn.f32x2 (one FADD2 per pair; a zero vector adds nothing)
+__device__ __forceinline__ void add_bf16x8(uint64_t (&acc)[4], const uint4 &v) {
+  acc[0] = add2(acc[0], pack2(__uint_as_float(v.x << 16), __uint_as_float(v.x & 0xffff0000u)));
+  acc[1] = add2(acc[1], pack2(__uint_as_float(v.y << 16), __uint_as_float(v.y & 0xffff0000u)));
+  acc[2] = add2(acc[2], pack2(__uint_as_float(v.z << 16), __uint_as_float(v.z & 0xffff0000u)));
+  acc[3] = add2(acc[3], pack2(__uint_as_float(v.w << 16), __uint_as_float(v.w & 0xffff0000u)));
 }
 
 constexpr int kPoolThreads = 256;
 
 // grid = (Nqb + Mmax, H, B).  blockIdx.x < Nqb: query block; otherwise historical K block m = x - Nqb.
+// One CTA reduces one block (<= 128 rows x d).  All of a thread's loads are issued before the first use; the per-row
+// address arithmetic is kept to a compare, a select and a multiply-add: the block's position in the logical sequence
+// is resolved ONCE per CTA (a 1-D block spans at most two pages when T_f >= block; a 3-D block's rows are shifts and
+// masks of the row index because bh * bw == 32).
 template <int D, bool K3D>
-__global__ void __launch_bounds__(kPoolThreads) li_pool_kernel(const SelectParams p, const BatchMeta meta) {
+__global__ void __launch_bounds__(kPoolThreads, 4) li_pool_kernel(const SelectParams p, const BatchMeta meta) {
   constexpr int TPR = D / 8;                 // threads per row (16-byte loads)
-  constexpr int RPP = kPoolThreads / TPR;    // rows per pass
-  constexpr int kMaxIter = 128 / RPP;        // passes for the largest block (128 rows); bf16 zero adds nothing
-  __shared__ float red[RPP][D];
+  constexpr int RPP = kPoolThreads / TPR;    // rows per pass (16 or 32: divides a 32-row frame slice)
+  constexpr int kMaxIter = 128 / RPP;        // passes for the largest block (128 rows)
+  __shared__ __align__(16) float red[RPP][D];
   pdl_launch_dependents();
   const int h = blockIdx.y, b = blockIdx.z;
   const int r0 = threadIdx.x / TPR, cofs = (threadIdx.x % TPR) * 8;
-  float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-  int nvalid;
-  float *out;
-  int out_stride = 1;
-
+  const bool is_q = (int)blockIdx.x < p.Nqb;
+  const int blk_id = is_q ? (int)blockIdx.x : (int)blockIdx.x - p.Nqb;
+  const int foff = meta.frame_off[b];
+  const int n_hist = meta.frame_off[b + 1] - foff - p.n_cur;
+  const int32_t *pages = p.frame_idx + foff;
   const Tiling tl = p.tl;
-  // 3-D blocks: row r of block m = (tg, hb, wb) is frame tg*bt + r/32, grid row hb*bh + (r%32)/bw,
-  // grid column wb*bw + (r%32)%bw; rows outside the grid or past the region's last frame are padding (not loaded,
-  // not counted: "masked loads").  Returns the token's row inside its frame, or -1 for padding.
-  auto row3d = [&](int m, int r, int n_reg, int &f) -> int {
-    const int per = tl.Hb * tl.Wb, tg = m / per, rem = m - tg * per, hb = rem / tl.Wb, wb = rem - hb * tl.Wb;
-    const int within = r & 31, hh = within / tl.bw, ww = within - hh * tl.bw;
-    f = tg * tl.bt + (r >> 5);
-    const int y = hb * tl.bh + hh;
-    return (f < n_reg && y < tl.gh) ? y * tl.gw + wb * tl.bw + ww : -1;
-  };
-  auto count3d = [&](int m, int n_reg) -> int {
-    const int per = tl.Hb * tl.Wb, tg = m / per, hb = (m - tg * per) / tl.Wb;
-    return min(tl.bt, n_reg - tg * tl.bt) * min(tl.bh, tl.gh - hb * tl.bh) * tl.bw;
+  if (!is_q && blk_id >= tl.num_blocks(n_hist, p.T_f, p.blk)) return;       // m >= M_b (whole CTA exits together)
+  const uint16_t *base = is_q ? p.q + b * p.q_sb + h * p.q_sh + cofs : p.k_cache + h * p.kv_sh + cofs;
+  const int64_t st = is_q ? p.q_st : p.kv_st;
+  // a page id outside the pool is never dereferenced: its rows count as zeros (li_validate reports the id)
+  auto page_base = [&](int f) -> const uint16_t * {
+    const int pg = __ldg(pages + f);
+    return (unsigned)pg < (unsigned)p.n_pages ? base + (int64_t)pg * p.kv_sp : nullptr;
   };
 
-  if ((int)blockIdx.x < p.Nqb) {
-    const int i = blockIdx.x;
-    uint4 v[kMaxIter];
-    if constexpr (K3D) {
-      const int n_reg = p.Lq / p.T_f;
-      nvalid = count3d(i, n_reg);
-      const uint16_t *base = p.q + b * p.q_sb + h * p.q_sh + cofs;
-#pragma unroll
-      for (int it = 0; it < kMaxIter; ++it) {
-        const int r = r0 + it * RPP;
-        int f;
-        const int row = r < p.blk ? row3d(i, r, n_reg, f) : -1;
-        v[it] = row >= 0 ? ldg_stream(base + ((int64_t)f * p.T_f + row) * p.q_st) : make_uint4(0, 0, 0, 0);
+  uint4 v[kMaxIter];
+  int nvalid;
+  if constexpr (K3D) {
+    // 3-D blocks: row r of block (tg, hb, wb) is frame tg*bt + r/32, grid row hb*bh + (r%32)/bw, grid
+    // column wb*bw + (r%32)%bw; rows outside the grid or past the region's last frame are padding (not loaded, not
+    // counted: "masked loads")
+    const int n_reg = is_q ? p.Lq / p.T_f : n_hist;
+    const int per = tl.Hb * tl.Wb, tg = blk_id / per, rem = blk_id - tg * per, hb = rem / tl.Wb, wb = rem - hb * tl.Wb;
+    const int nf = min(tl.bt, n_reg - tg * tl.bt), vh = min(tl.bh, tl.gh - hb * tl.bh), vw = min(tl.bw, tl.gw - wb * tl.bw);
+    nvalid = nf * vh * vw;
+    if (!is_q && p.slice_cache != nullptr) {
+      // page-resident patch sums (li_pool_pages): the block mean from <= bt cached rows, one channel per thread
+      if (threadIdx.x < D) {
+        float s = 0.f;
+        for (int f = 0; f < nf; ++f) {
+          const int pg = __ldg(pages + tg * tl.bt + f);
+          if ((unsigned)pg < (unsigned)p.n_pages) s += __ldg(p.slice_cache + (((int64_t)pg * p.H + h) * per + rem) * D + threadIdx.x);
+        }
+        p.kbar[(((int64_t)b * p.H + h) * D + threadIdx.x) * p.Mp + blk_id] = s / (float)nvalid;
       }
-    } else {
-      const int t0 = i * p.blk;
-      nvalid = min(p.blk, p.Lq - t0);
-      const uint16_t *base = p.q + b * p.q_sb + h * p.q_sh + (int64_t)t0 * p.q_st + cofs;
-#pragma unroll
-      for (int it = 0; it < kMaxIter; ++it) {
-        const int r = r0 + it * RPP;
-        v[it] = r < nvalid ? ldg_stream(base + (int64_t)r * p.q_st) : make_uint4(0, 0, 0, 0);
-      }
+      return;
     }
 #pragma unroll
-    for (int it = 0; it < kMaxIter; ++it) add_bf16x8(acc, v[it]);
-    out = p.qbar + (((int64_t)b * p.H + h) * p.Nqb + i) * D;
-  } else {
-    const int m = blockIdx.x - p.Nqb;
-    const int foff = meta.frame_off[b];
-    const int n_hist = meta.frame_off[b + 1] - foff - p.n_cur;
-    if (m >= tl.num_blocks(n_hist, p.T_f, p.blk)) return;          // m >= M_b (whole CTA exits together)
-    const uint16_t *base = p.k_cache + h * p.kv_sh + cofs;
-    const int32_t *pages = p.frame_idx + foff;
-    uint4 v[kMaxIter];
-    if constexpr (K3D) {
-      nvalid = count3d(m, n_hist);
-      if (p.slice_cache != nullptr) {
-        // page-resident patch sums (li_pool_pages): the block mean from <= bt cached rows, one channel per thread
-        if (threadIdx.x < D) {
-          const int per = tl.Hb * tl.Wb, tg = m / per, patch = m - tg * per;
-          const int nf = min(tl.bt, n_hist - tg * tl.bt);
-          float s = 0.f;
-          for (int f = 0; f < nf; ++f)
-            s += __ldg(p.slice_cache + (((int64_t)__ldg(pages + tg * tl.bt + f) * p.H + h) * per + patch) * D + threadIdx.x);
-          p.kbar[(((int64_t)b * p.H + h) * D + threadIdx.x) * p.Mp + m] = s / (float)nvalid;
-        }
-        return;
+    for (int it = 0; it < kMaxIter; ++it) {
+      const int fs = (it * RPP) >> 5;                                       // frame slice of this pass (compile time)
+      const int within = r0 + ((it * RPP) & 31), hh = within >> tl.bw_log2, ww = within & (tl.bw - 1);
+      v[it] = make_uint4(0, 0, 0, 0);
+      if (fs < nf && hh < vh && ww < vw) {
+        const int f = tg * tl.bt + fs;
+        const uint16_t *fb = is_q ? base + (int64_t)f * p.T_f * st : page_base(f);
+        if (fb != nullptr) v[it] = ldg_stream(fb + (int64_t)((hb * tl.bh + hh) * tl.gw + wb * tl.bw + ww) * st);
       }
+    }
+  } else {
+    const int L = is_q ? p.Lq : n_hist * p.T_f, t0 = blk_id * p.blk;
+    nvalid = min(p.blk, L - t0);
+    if (is_q) {
+      const uint16_t *b0 = base + (int64_t)t0 * st;
 #pragma unroll
       for (int it = 0; it < kMaxIter; ++it) {
         const int r = r0 + it * RPP;
-        int f;
-        const int row = r < p.blk ? row3d(m, r, n_hist, f) : -1;
-        v[it] = make_uint4(0, 0, 0, 0);
-        if (row >= 0) v[it] = ldg_stream(base + __ldg(pages + f) * p.kv_sp + row * p.kv_st);
+        v[it] = r < nvalid ? ldg_stream(b0 + (int64_t)r * st) : make_uint4(0, 0, 0, 0);
+      }
+    } else if (p.T_f >= p.blk) {
+      // the block touches at most two pages: rows [0, split) lie in page F[pg0], the rest in page F[pg0 + 1]
+      const int pg0 = t0 / p.T_f, row0 = t0 - pg0 * p.T_f, split = p.T_f - row0;
+      const uint16_t *b0 = page_base(pg0), *b1 = split < nvalid ? page_base(pg0 + 1) : nullptr;
+      if (b0 != nullptr) b0 += (int64_t)row0 * st;
+      if (b1 != nullptr) b1 -= (int64_t)split * st;
+#pragma unroll
+      for (int it = 0; it < kMaxIter; ++it) {
+        const int r = r0 + it * RPP;
+        const uint16_t *rb = r < split ? b0 : b1;
+        v[it] = (r < nvalid && rb != nullptr) ? ldg_stream(rb + (int64_t)r * st) : make_uint4(0, 0, 0, 0);
       }
     } else {
-      const int L_hist = n_hist * p.T_f;
-      const int t0 = m * p.blk;
-      nvalid = min(p.blk, L_hist - t0);
+      // frames shorter than a block: one page lookup per row
 #pragma unroll
       for (int it = 0; it < kMaxIter; ++it) {
         const int r = r0 + it * RPP;
         v[it] = make_uint4(0, 0, 0, 0);
         if (r < nvalid) {
-          const int t = t0 + r;
-          const int pg = t / p.T_f;
-          const int row = t - pg * p.T_f;
-          const int page = __ldg(pages + pg);
-          v[it] = ldg_stream(base + page * p.kv_sp + row * p.kv_st);
+          const int t = t0 + r, pg = t / p.T_f;
+          const uint16_t *rb = page_base(pg);
+          if (rb != nullptr) v[it] = ldg_stream(rb + (int64_t)(t - pg * p.T_f) * st);
         }
       }
     }
-#pragma unroll
-    for (int it = 0; it < kMaxIter; ++it) add_bf16x8(acc, v[it]);
-    out = p.kbar + ((int64_t)b * p.H + h) * D * p.Mp + m;          // kbar is stored TRANSPOSED: [B,H,d,Mp]
-    out_stride = p.Mp;
   }
-
+  uint64_t acc[4] = {0ull, 0ull, 0ull, 0ull};                              // four (+0.0f, +0.0f) pairs
 #pragma unroll
-  for (int e = 0; e < 8; ++e) red[r0][cofs + e] = acc[e];
+  for (int it = 0; it < kMaxIter; ++it) add_bf16x8(acc, v[it]);
+
+  *reinterpret_cast<uint4 *>(&red[r0][cofs]) = make_uint4((uint32_t)acc[0], (uint32_t)(acc[0] >> 32), (uint32_t)acc[1], (uint32_t)(acc[1] >> 32));
+  *reinterpret_cast<uint4 *>(&red[r0][cofs + 4]) = make_uint4((uint32_t)acc[2], (uint32_t)(acc[2] >> 32), (uint32_t)acc[3], (uint32_t)(acc[3] >> 32));
   __syncthreads();
   if (threadIdx.x < D) {
     float s = 0.f;
 #pragma unroll
     for (int r = 0; r < RPP; ++r) s += red[r][threadIdx.x];
-    out[(int64_t)threadIdx.x * out_stride] = s / (float)nvalid;    // Eq. 9: true cardinality |Q_i|, |K_m|
+    const float mean = s / (float)nvalid;                                    // Eq. 9: true cardinality |Q_i|, |K_m|
+    if (is_q) p.qbar[(((int64_t)b * p.H + h) * p.Nqb + blk_id) * D + threadIdx.x] = mean;
+    else p.kbar[(((int64_t)b * p.H + h) * D + threadIdx.x) * p.Mp + blk_id] = mean;   // kbar is stored TRANSPOSED: [B,H,d,Mp]
   }
 }
-
-constexpr int kRowsPerWarp = 8;              // query-block rows scored together by one warp
-constexpr int kKeysPerLane = 16;             // top-k register fast path covers M <= 512 historical blocks
-constexpr int kTopkWarps = 8;                // rows (warps) per CTA of the top-k kernel
 
 __device__ __forceinline__ uint32_t order_key(float s) {
   const uint32_t u = __float_as_uint(s);
   return (u & 0x80000000u) ? ~u : (u | 0x80000000u);   // unsigned order == float order
 }
 
-// Scores (Eq. 10).  grid = (ceil(Mmax/32), ceil(Nqb/8), B*H), 4 warps per CTA.  The work is latency-bound (a few MFLOP
-// spread over thousands of CTAs), so the dependent chain of every warp is kept short: lane = one historical block m,
-// warp w walks channels [w*D/4, (w+1)*D/4) of its pooled key row (one coalesced 128-byte line per channel, kbar is
-// channel-major) against 8 pooled query rows broadcast from shared memory = 8 independent fp32 FMA chains; the 4
-// partial sums of a score are added in a fixed order (w = 0..3) through shared memory.  Output: order-preserving keys
-// [B,H,Nqb,Mmax] (+ scores).
+// ----------------------------------------------------------------------------- fused scores + Top_k (Eq. 10), M <= 512
+// One CTA = 8 consecutive query-block rows of one (call, head); grid = (ceil(Nqb / 8), B*H), 8 warps.
+// Phase 1 (scores): warp w = (row half rh = w / 4, channel quarter cq = w % 4) accumulates, for its 4 rows, the partial
+//   dot products over channels [cq*D/4, (cq+1)*D/4): lane = historical block m = lane + 32 x, x < NX, i.e. 4 * NX
+//   independent fp32 FMA chains per lane; kbar is channel-major, so for a fixed channel the 32 lanes read one 128-byte
+//   line and every loaded value feeds 4 FMAs; the pooled query rows are broadcast from shared memory.  The loads of the
+//   next channel pair are issued before the FMAs of the current one.  Partials -> shared memory [cq][row][Mp].
+// Phase 2 (Top_k): warp w owns row w: the 4 partial sums of a score are added in a fixed order (cq = 0..3), the scores
+//   stay in registers as order-preserving keys, the k-th largest is found by an MSB-first radix select (32 counting
+//   passes with redux.sync), and one ordered pass emits, ascending, every block above the threshold plus the
+//   lowest-index blocks equal to it.
+constexpr int kSelRows = 8;
+template <int D, int NX>
+__global__ void __launch_bounds__(kSelRows * 32) li_score_topk_kernel(const SelectParams p, const BatchMeta meta) {
+  extern __shared__ __align__(16) float sel_smem[];
+  constexpr int DW = D / 4;                                // channels per warp
+  float *sq = sel_smem;                                    // [8 rows][D]
+  float *part = sel_smem + kSelRows * D;                   // [4 quarters][8 rows][Mp]
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int bh = blockIdx.y, b = bh / p.H;
+  const int i0 = blockIdx.x * kSelRows;
+  const int n_hist = meta.frame_off[b + 1] - meta.frame_off[b] - p.n_cur;
+  const int M = p.tl.num_blocks(n_hist, p.T_f, p.blk);
+  const int k = min(meta.top_k[b], M);
+  const int nx = (M + 31) >> 5;                            // 32-block groups that exist (CTA-uniform)
+  pdl_launch_dependents();
+  pdl_wait();                                              // qbar / kbar come from li_pool_kernel
+
+  if (M > 0 && (k > 0 || p.scores != nullptr)) {
+    for (int t = threadIdx.x; t < kSelRows * D / 4; t += kSelRows * 32) {
+      const int g = t / (D / 4);
+      reinterpret_cast<float4 *>(sq)[t] =
+          (i0 + g < p.Nqb) ? __ldg(reinterpret_cast<const float4 *>(p.qbar + ((int64_t)bh * p.Nqb + i0) * D) + t)
+                           : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    const int rh = warp >> 2, cq = warp & 3;
+    const float *kT = p.kbar + ((int64_t)bh * D + cq * DW) * p.Mp + lane;   // lanes past M read the row's padding; dropped
+    float acc[4][NX];
+#pragma unroll
+    for (int r = 0; r < 4; ++r)
+#pragma unroll
+      for (int x = 0; x < NX; ++x) acc[r][x] = 0.f;
+    float kv[2][2][NX];                                    // [buffer][channel of the pair][group]
+    auto load_pair = [&](int buf, int c) {
+#pragma unroll
+      for (int cc = 0; cc < 2; ++cc)
+#pragma unroll
+        for (int x = 0; x < NX; ++x) kv[buf][cc][x] = x < nx ? __ldg(kT + (int64_t)(c + cc) * p.Mp + 32 * x) : 0.f;
+    };
+    auto fma_pair = [&](int buf, int c) {
+#pragma unroll
+      for (int cc = 0; cc < 2; ++cc)
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+          const float qc = sq[(rh * 4 + r) * D + cq * DW + c + cc];
+#pragma unroll
+          for (int x = 0; x < NX; ++x) acc[r][x] = fmaf(qc, kv[buf][cc][x], acc[r][x]);
+        }
+    };
+    load_pair(0, 0);
+    __syncthreads();                                       // sq staged
+#pragma unroll 1
+    for (int c = 0; c < DW; c += 4) {
+      load_pair(1, c + 2);
+      fma_pair(0, c);
+      if (c + 4 < DW) load_pair(0, c + 4);
+      fma_pair(1, c + 2);
+    }
+#pragma unroll
+    for (int r = 0; r < 4; ++r)
+#pragma unroll
+      for (int x = 0; x < NX; ++x)
+        if (x < nx) part[((size_t)cq * kSelRows + rh * 4 + r) * p.Mp + lane + 32 * x] = acc[r][x];
+  }
+  __syncthreads();
+
+  const int i = i0 + warp;
+  if (i >= p.Nqb) return;                                  // whole warp; no CTA-wide barrier below
+  const int64_t row = (int64_t)bh * p.Nqb + i;
+  int32_t *out = p.sel_idx + row * p.kmax;
+  if (lane == 0) p.sel_cnt[row] = k;
+  uint32_t kr[NX];
+#pragma unroll
+  for (int x = 0; x < NX; ++x) {
+    const int m = lane + 32 * x;
+    kr[x] = 0u;                                            // absent blocks: key 0, below every real key
+    if (m < M && (k > 0 || p.scores != nullptr)) {
+      const float *pr = part + (size_t)warp * p.Mp + m;
+      const size_t qs = (size_t)kSelRows * p.Mp;
+      const float dot = ((pr[0] + pr[qs]) + pr[2 * qs]) + pr[3 * qs];
+      const float sc = dot * p.inv_sqrt_d + 0.0f;          // -0 -> +0 so that equal scores have equal keys
+      kr[x] = order_key(sc);
+      if (p.scores != nullptr) p.scores[row * p.score_pitch + m] = sc;
+    }
+  }
+  if (k > 0) {
+    // T = k-th largest key: built MSB first, keeping count(key >= T) >= k
+    uint32_t T = 0;
+    for (int bit = 31; bit >= 0; --bit) {
+      const uint32_t cand = T | (1u << bit);
+      int c = 0;
+#pragma unroll
+      for (int x = 0; x < NX; ++x) c += kr[x] >= cand;
+      c = __reduce_add_sync(0xffffffffu, c);
+      if (c >= k) T = cand;
+    }
+    int c_gt = 0;
+#pragma unroll
+    for (int x = 0; x < NX; ++x) c_gt += kr[x] > T;
+    c_gt = __reduce_add_sync(0xffffffffu, c_gt);
+    int need_eq = k - c_gt;                                // ties at the threshold: lowest index first
+    int pos = 0;
+    const uint32_t lt = (1u << lane) - 1u;
+#pragma unroll
+    for (int x = 0; x < NX; ++x) {
+      const bool gt = kr[x] > T;
+      const bool eq = kr[x] == T && T != 0u;
+      const uint32_t eq_mask = __ballot_sync(0xffffffffu, eq);
+      const bool take = gt || (eq && __popc(eq_mask & lt) < need_eq);
+      const uint32_t take_mask = __ballot_sync(0xffffffffu, take);
+      if (take) out[pos + __popc(take_mask & lt)] = lane + 32 * x;
+      pos += __popc(take_mask);
+      need_eq -= min(need_eq, __popc(eq_mask));
+    }
+  }
+  for (int t = k + lane; t < p.kmax; t += 32) out[t] = -1;
+}
+
+// ----------------------------------------------------------------------------- M > 512: scores and Top_k as two launches
+constexpr int kRowsPerWarp = 8;              // query-block rows scored together by one warp
+constexpr int kTopkWarps = 8;                // rows (warps) per CTA of the top-k kernel
 constexpr int kScoreWarps = 4;
+// grid = (ceil(Mmax/32), ceil(Nqb/8), B*H), 4 warps per CTA: lane = one historical block m, warp w walks channels
+// [w*D/4, (w+1)*D/4) against 8 pooled query rows broadcast from shared memory; the 4 partial sums of a score are added
+// in a fixed order through shared memory.  Output: order-preserving keys [B,H,Nqb,Mmax] (+ scores).
 template <int D>
 __global__ void __launch_bounds__(kScoreWarps * 32) li_score_kernel(const SelectParams p, const BatchMeta meta) {
   __shared__ __align__(16) float sq[kRowsPerWarp * D];
@@ -186,8 +304,6 @@ __global__ void __launch_bounds__(kScoreWarps * 32) li_score_kernel(const Select
   pdl_launch_dependents();
   pdl_wait();                                              // qbar / kbar come from li_pool_kernel
 
-  // kbar is [B,H,d,Mp] (written transposed by the pool kernel): for a fixed channel the 32 lanes read 32
-  // consecutive floats = one 128-byte line.  Lanes past M read padding and their results are dropped.
   constexpr int DW = D / kScoreWarps;                        // channels per warp
   const float *kT = p.kbar + ((int64_t)bh * D + warp * DW) * p.Mp + m;
   float kv[DW];
@@ -232,9 +348,7 @@ __global__ void __launch_bounds__(kScoreWarps * 32) li_score_kernel(const Select
   }
 }
 
-// Top_k (Eq. 10).  One warp per (call, head, query block) row; grid = ceil(B*H*Nqb / 8) CTAs of 8 warps.
-// MSB-first radix select of the k-th largest key, then one ordered pass that emits, ascending, every block above
-// the threshold plus the lowest-index blocks equal to it.
+// One warp per row; grid = ceil(B*H*Nqb / 8) CTAs of 8 warps; keys re-read from the workspace in every counting pass.
 __global__ void __launch_bounds__(kTopkWarps * 32) li_topk_kernel(const SelectParams p, const BatchMeta meta) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int64_t row = (int64_t)blockIdx.x * kTopkWarps + warp;
@@ -249,65 +363,31 @@ __global__ void __launch_bounds__(kTopkWarps * 32) li_topk_kernel(const SelectPa
   int32_t *out = p.sel_idx + row * p.kmax;
   if (lane == 0) p.sel_cnt[row] = k;
   if (k > 0) {
-    // T = k-th largest key: build it MSB first, keeping count(key >= T) >= k
     uint32_t T = 0;
     int c_gt = 0;
-    if (M <= 32 * kKeysPerLane) {
-      // fast path: each lane keeps its keys (block m = lane + 32*x) in registers; absent blocks get key 0,
-      // which is below every real key (order_key never returns 0 for a non-NaN score)
-      uint32_t kr[kKeysPerLane];
-#pragma unroll
-      for (int x = 0; x < kKeysPerLane; ++x) kr[x] = (lane + 32 * x < M) ? key[lane + 32 * x] : 0u;
-      for (int bit = 31; bit >= 0; --bit) {
-        const uint32_t cand = T | (1u << bit);
-        int c = 0;
-#pragma unroll
-        for (int x = 0; x < kKeysPerLane; ++x) c += kr[x] >= cand;
-        c = __reduce_add_sync(0xffffffffu, c);
-        if (c >= k) T = cand;
-      }
-#pragma unroll
-      for (int x = 0; x < kKeysPerLane; ++x) c_gt += kr[x] > T;
-      c_gt = __reduce_add_sync(0xffffffffu, c_gt);
-      int need_eq = k - c_gt;                                // ties at the threshold: lowest index first
-      int pos = 0;
-#pragma unroll
-      for (int x = 0; x < kKeysPerLane; ++x) {
-        const bool gt = kr[x] > T;
-        const bool eq = kr[x] == T && T != 0u;
-        const uint32_t eq_mask = __ballot_sync(0xffffffffu, eq);
-        const uint32_t lt = (1u << lane) - 1u;
-        const bool take = gt || (eq && __popc(eq_mask & lt) < need_eq);
-        const uint32_t take_mask = __ballot_sync(0xffffffffu, take);
-        if (take) out[pos + __popc(take_mask & lt)] = lane + 32 * x;
-        pos += __popc(take_mask);
-        need_eq -= min(need_eq, __popc(eq_mask));
-      }
-    } else {
-      for (int bit = 31; bit >= 0; --bit) {
-        const uint32_t cand = T | (1u << bit);
-        int c = 0;
-        for (int m = lane; m < M; m += 32) c += key[m] >= cand;
-        c = __reduce_add_sync(0xffffffffu, c);
-        if (c >= k) T = cand;
-      }
-      for (int m = lane; m < M; m += 32) c_gt += key[m] > T;
-      c_gt = __reduce_add_sync(0xffffffffu, c_gt);
-      int need_eq = k - c_gt;
-      int pos = 0;
-      for (int m0 = 0; m0 < M; m0 += 32) {
-        const int m = m0 + lane;
-        const uint32_t kv = m < M ? key[m] : 0u;
-        const bool gt = m < M && kv > T;
-        const bool eq = m < M && kv == T;
-        const uint32_t eq_mask = __ballot_sync(0xffffffffu, eq);
-        const uint32_t lt = (1u << lane) - 1u;
-        const bool take = gt || (eq && __popc(eq_mask & lt) < need_eq);
-        const uint32_t take_mask = __ballot_sync(0xffffffffu, take);
-        if (take) out[pos + __popc(take_mask & lt)] = m;
-        pos += __popc(take_mask);
-        need_eq -= min(need_eq, __popc(eq_mask));
-      }
+    for (int bit = 31; bit >= 0; --bit) {
+      const uint32_t cand = T | (1u << bit);
+      int c = 0;
+      for (int m = lane; m < M; m += 32) c += key[m] >= cand;
+      c = __reduce_add_sync(0xffffffffu, c);
+      if (c >= k) T = cand;
+    }
+    for (int m = lane; m < M; m += 32) c_gt += key[m] > T;
+    c_gt = __reduce_add_sync(0xffffffffu, c_gt);
+    int need_eq = k - c_gt;
+    int pos = 0;
+    for (int m0 = 0; m0 < M; m0 += 32) {
+      const int m = m0 + lane;
+      const uint32_t kv = m < M ? key[m] : 0u;
+      const bool gt = m < M && kv > T;
+      const bool eq = m < M && kv == T;
+      const uint32_t eq_mask = __ballot_sync(0xffffffffu, eq);
+      const uint32_t lt = (1u << lane) - 1u;
+      const bool take = gt || (eq && __popc(eq_mask & lt) < need_eq);
+      const uint32_t take_mask = __ballot_sync(0xffffffffu, take);
+      if (take) out[pos + __popc(take_mask & lt)] = m;
+      pos += __popc(take_mask);
+      need_eq -= min(need_eq, __popc(eq_mask));
     }
   }
   for (int t = k + lane; t < p.kmax; t += 32) out[t] = -1;
@@ -322,20 +402,21 @@ template <int D>
 __global__ void __launch_bounds__(128) li_pool_pages_kernel(const SelectParams p, const int32_t *pages, float *cache) {
   constexpr int TPR = D / 8;                 // threads per row (16-byte loads)
   constexpr int RPP = 128 / TPR;             // rows per pass
-  __shared__ float red[RPP][D];
+  __shared__ __align__(16) float red[RPP][D];
   const Tiling tl = p.tl;
   const int patch = blockIdx.x, h = blockIdx.y, page = pages[blockIdx.z];
+  if ((unsigned)page >= (unsigned)p.n_pages) return;                        // never read or written (li_validate reports it)
   const int hb = patch / tl.Wb, wb = patch - hb * tl.Wb;
   const int r0 = threadIdx.x / TPR, cofs = (threadIdx.x % TPR) * 8;
-  float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  uint64_t acc[4] = {0ull, 0ull, 0ull, 0ull};
   const uint16_t *base = p.k_cache + (int64_t)page * p.kv_sp + h * p.kv_sh + cofs;
 #pragma unroll
   for (int it = 0; it < 32 / RPP; ++it) {
-    const int r = r0 + it * RPP, hh = r / tl.bw, ww = r - hh * tl.bw, y = hb * tl.bh + hh;
-    if (y < tl.gh) add_bf16x8(acc, ldg_stream(base + (int64_t)(y * tl.gw + wb * tl.bw + ww) * p.kv_st));
+    const int r = r0 + it * RPP, hh = r >> tl.bw_log2, ww = r & (tl.bw - 1), y = hb * tl.bh + hh, x = wb * tl.bw + ww;
+    if (y < tl.gh && x < tl.gw) add_bf16x8(acc, ldg_stream(base + (int64_t)(y * tl.gw + x) * p.kv_st));
   }
-#pragma unroll
-  for (int e = 0; e < 8; ++e) red[r0][cofs + e] = acc[e];
+  *reinterpret_cast<uint4 *>(&red[r0][cofs]) = make_uint4((uint32_t)acc[0], (uint32_t)(acc[0] >> 32), (uint32_t)acc[1], (uint32_t)(acc[1] >> 32));
+  *reinterpret_cast<uint4 *>(&red[r0][cofs + 4]) = make_uint4((uint32_t)acc[2], (uint32_t)(acc[2] >> 32), (uint32_t)acc[3], (uint32_t)(acc[3] >> 32));
   __syncthreads();
   if (threadIdx.x < D) {
     float s = 0.f;
@@ -352,6 +433,34 @@ int launch_pool_pages(const SelectParams &sp, const int32_t *pages, int n_list, 
   else li_pool_pages_kernel<64><<<grid, 128, 0, st>>>(sp, pages, cache);
   if (n_launches) *n_launches += 1;
   return (int)cudaGetLastError();
+}
+
+template <int D, int NX>
+static cudaError_t launch_score_topk_nx(cudaLaunchConfig_t &cfg, const SelectParams &sp, const BatchMeta &meta) {
+  // shared memory: 8 pooled query rows + the partial sums [4][8][Mp]; above 48 KB the limit is raised once per device
+  cfg.dynamicSmemBytes = (size_t)(kSelRows * D + 4 * kSelRows * sp.Mp) * sizeof(float);
+  if (cfg.dynamicSmemBytes > 48 * 1024) {
+    static std::atomic<uint64_t> attr_done{0};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const uint64_t dev_bit = 1ull << (dev & 63);
+    if (!(attr_done.load(std::memory_order_acquire) & dev_bit)) {
+      e = cudaFuncSetAttribute(li_score_topk_kernel<D, NX>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               (kSelRows * D + 4 * kSelRows * 512) * (int)sizeof(float));
+      if (e != cudaSuccess) return e;
+      attr_done.fetch_or(dev_bit, std::memory_order_release);
+    }
+  }
+  return cudaLaunchKernelEx(&cfg, li_score_topk_kernel<D, NX>, sp, meta);
+}
+template <int D>
+static cudaError_t launch_score_topk(cudaLaunchConfig_t &cfg, const SelectParams &sp, const BatchMeta &meta) {
+  if (sp.Mmax <= 128) return launch_score_topk_nx<D, 4>(cfg, sp, meta);
+  if (sp.Mmax <= 192) return launch_score_topk_nx<D, 6>(cfg, sp, meta);
+  if (sp.Mmax <= 256) return launch_score_topk_nx<D, 8>(cfg, sp, meta);
+  if (sp.Mmax <= 384) return launch_score_topk_nx<D, 12>(cfg, sp, meta);
+  return launch_score_topk_nx<D, 16>(cfg, sp, meta);
 }
 
 int launch_select(const SelectParams &sp, const BatchMeta &meta, cudaStream_t st, int64_t *n_launches) {
@@ -371,13 +480,21 @@ int launch_select(const SelectParams &sp, const BatchMeta &meta, cudaStream_t st
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
-  if (sp.Mmax > 0) {
-    cudaLaunchConfig_t cfg = {};
+  cudaLaunchConfig_t cfg = {};
+  cfg.stream = st;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  if (sp.Mmax <= 512) {
+    cfg.gridDim = dim3((sp.Nqb + kSelRows - 1) / kSelRows, sp.B * sp.H);
+    cfg.blockDim = dim3(kSelRows * 32);
+    cudaError_t e = sp.d == 128 ? launch_score_topk<128>(cfg, sp, meta) : launch_score_topk<64>(cfg, sp, meta);
+    if (e != cudaSuccess) return (int)e;
+    if (n_launches) *n_launches += 1;
+    return 0;
+  }
+  {
     cfg.gridDim = dim3((sp.Mmax + 31) / 32, (sp.Nqb + kRowsPerWarp - 1) / kRowsPerWarp, sp.B * sp.H);
     cfg.blockDim = dim3(kScoreWarps * 32);
-    cfg.stream = st;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
     cudaError_t e = sp.d == 128 ? cudaLaunchKernelEx(&cfg, li_score_kernel<128>, sp, meta)
                                 : cudaLaunchKernelEx(&cfg, li_score_kernel<64>, sp, meta);
     if (e != cudaSuccess) return (int)e;
@@ -385,17 +502,68 @@ int launch_select(const SelectParams &sp, const BatchMeta &meta, cudaStream_t st
   }
   {
     const int64_t rows = (int64_t)sp.B * sp.H * sp.Nqb;
-    cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)((rows + kTopkWarps - 1) / kTopkWarps));
     cfg.blockDim = dim3(kTopkWarps * 32);
-    cfg.stream = st;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
     cudaError_t e = cudaLaunchKernelEx(&cfg, li_topk_kernel, sp, meta);
     if (e != cudaSuccess) return (int)e;
     if (n_launches) *n_launches += 1;
   }
   return 0;
+}
+
+// ----------------------------------------------------------------------------- li_validate (debug, include/li.h)
+// CTAs [0, n_list_ctas): 256 frame-list entries each.  Then one CTA per (call, head, query block) row of sel_idx:
+// count and range checks, duplicates through a bitmap of M bits in shared memory.
+__device__ __forceinline__ void report(int32_t *err, int bit, int b, int pos, int val) {
+  atomicOr(&err[0], bit);
+  if (atomicCAS(&err[1], 0, b + 1) == 0) { err[2] = pos; err[3] = val; }
+}
+constexpr int kBitmapWords = 8192;          // duplicates are checked for M <= 262144
+__global__ void __launch_bounds__(256) li_validate_kernel(const ValidateParams v, const BatchMeta meta, int n_list_ctas) {
+  __shared__ uint32_t bm[kBitmapWords];
+  if ((int)blockIdx.x < n_list_ctas) {
+    const int e = blockIdx.x * 256 + threadIdx.x;
+    if (e < meta.frame_off[v.B]) {
+      const int pg = v.frame_idx[e];
+      if ((unsigned)pg >= (unsigned)v.n_pages) {
+        int b = 0;
+        while (b + 1 < v.B && meta.frame_off[b + 1] <= e) ++b;
+        report(v.err, LI_BAD_PAGE_ID, b, e, pg);
+      }
+    }
+    return;
+  }
+  const int64_t row = (int64_t)blockIdx.x - n_list_ctas;
+  const int b = (int)(row / ((int64_t)v.H * v.Nqb));
+  const int n_hist = meta.frame_off[b + 1] - meta.frame_off[b] - v.n_cur;
+  const int M = v.tl.num_blocks(n_hist, v.T_f, v.blk);
+  const int cnt = v.sel_cnt[row];
+  const int pos0 = (int)((row - (int64_t)b * v.H * v.Nqb) * v.kmax);
+  if (cnt < 0 || cnt > v.kmax || cnt > M) {
+    if (threadIdx.x == 0) report(v.err, LI_BAD_SEL_CNT, b, (int)(row - (int64_t)b * v.H * v.Nqb), cnt);
+    return;
+  }
+  const bool dup_check = M <= kBitmapWords * 32;
+  if (dup_check)
+    for (int w = threadIdx.x; w < (M + 31) / 32; w += 256) bm[w] = 0u;
+  __syncthreads();
+  const int32_t *sel = v.sel_idx + row * v.kmax;
+  for (int t = threadIdx.x; t < cnt; t += 256) {
+    const int m = sel[t];
+    if (m < 0 || m >= M) report(v.err, LI_BAD_SEL_RANGE, b, pos0 + t, m);
+    else if (dup_check && (atomicOr(&bm[m >> 5], 1u << (m & 31)) >> (m & 31)) & 1u) report(v.err, LI_BAD_SEL_DUPLICATE, b, pos0 + t, m);
+  }
+}
+
+int launch_validate(const ValidateParams &vp, const BatchMeta &meta, cudaStream_t st, int64_t *n_launches) {
+  cudaError_t e = cudaMemsetAsync(vp.err, 0, 4 * sizeof(int32_t), st);
+  if (e != cudaSuccess) return (int)e;
+  const int n_list_ctas = (meta.frame_off[vp.B] + 255) / 256;
+  const int64_t rows = vp.sel_idx != nullptr ? (int64_t)vp.B * vp.H * vp.Nqb : 0;
+  if (n_list_ctas + rows == 0) return 0;
+  li_validate_kernel<<<(unsigned)(n_list_ctas + rows), 256, 0, st>>>(vp, meta, n_list_ctas);
+  if (n_launches) *n_launches += 1;
+  return (int)cudaGetLastError();
 }
 
 }  // namespace li

@@ -16,18 +16,18 @@ MAX_ABS, MEAN_ABS = 2e-2, 2e-3
 LSE_ABS = 2e-3   # fp32 online softmax vs fp64 two-pass; logits are O(10), ex2.approx/log2 rel. error ~1e-6..1e-7
 
 
-def upload(prob: W.Problem, dev="cuda:0"):
+def upload(prob: W.Problem, dev="cuda:0", flags=0):
     q = prob.q.to(dev)
     kc = prob.k_cache.to(dev)
     vc = prob.v_cache.to(dev)
     fi = torch.from_numpy(prob.frame_idx).to(dev)
     ctx = li.Context(q, kc, vc, fi, prob.frame_off, prob.spec.n_cur_frames, prob.spec.block,
-                     grid=prob.spec.grid, block3d=prob.spec.block3d)
+                     grid=prob.spec.grid, block3d=prob.spec.block3d, flags=flags)
     return ctx
 
 
-def run_gpu(prob: W.Problem, want_scores=True, kmax=None):
-    ctx = upload(prob)
+def run_gpu(prob: W.Problem, want_scores=True, kmax=None, flags=0):
+    ctx = upload(prob, flags=flags)
     buf = li.Buffers(ctx, kmax if kmax is not None else prob.kmax, want_scores=want_scores)
     buf.sel_idx.fill_(-7)
     buf.o.fill_(float("nan"))

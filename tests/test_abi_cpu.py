@@ -30,7 +30,7 @@ def test_every_declared_symbol_is_exported(L):
     assert set(names) == set(li.EXPORTS)
     for n in names:
         assert getattr(L, n) is not None
-    assert li.version() == 102
+    assert li.version() == 200
     assert li.strerror(0) == "ok" and "unsupported" in li.strerror(li.LI_ERR_UNSUPPORTED)
 
 
@@ -204,3 +204,51 @@ def test_slice_cache_validation(L):
     ws3 = L.li_workspace_bytes(ctypes.byref(p3), 8)
     assert L.li_block_select_cached(ctypes.byref(p3), tk.ctypes.data, 8, 0x60000, 0x70000, None, 0, 0, 0x50000, ws3,
                                     None) == li.LI_ERR_INVALID_ARG
+
+
+def test_validate_and_flags_argument_checks(L):
+    """li_validate (debug check of device-side inputs) and li_problem.flags: host-side rejections."""
+    p, fo = make_problem()
+    assert L.li_validate(ctypes.byref(p), None, None, 0, None, None) == li.LI_ERR_INVALID_ARG          # no error word
+    assert L.li_validate(ctypes.byref(p), 0x60000, None, 8, 0x90000, None) == li.LI_ERR_INVALID_ARG    # sel_idx without sel_cnt
+    assert L.li_validate(ctypes.byref(p), None, 0x70000, 8, 0x90000, None) == li.LI_ERR_INVALID_ARG
+    assert L.li_validate(ctypes.byref(p), 0x60000, 0x70000, 0, 0x90000, None) == li.LI_ERR_INVALID_ARG  # kmax < 1
+    bad, keep = make_problem(d=96)
+    assert L.li_validate(ctypes.byref(bad), None, None, 0, 0x90000, None) == li.LI_ERR_UNSUPPORTED
+    assert li.LI_FLAG_NO_SPLIT == 1 and li.li_problem.flags.size == 4
+    # the struct mirrors include/li.h field for field (flags is the last member)
+    hdr = open(os.path.join(ROOT, "include", "li.h")).read()
+    body = hdr[hdr.index("typedef struct li_problem {"):hdr.index("} li_problem;")]
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    names = []
+    for decl in body.split(";"):
+        decl = decl.replace("typedef struct li_problem {", "").strip()
+        if decl:
+            names += [n.strip().lstrip("*").strip() for n in re.sub(r"^(const\s+)?\w+(\s+\*?|\s*\*\s*)", "", decl, count=1).split(",")]
+    assert names == [f[0] for f in li.li_problem._fields_]
+
+
+def test_page_pool_entry_points_need_only_the_cache(L):
+    """li_slice_cache_bytes / li_pool_pages look at the K cache and the tiling only: Q, the frame lists and their host
+    offsets may be absent."""
+    p3, keep3 = make_problem(frame_tokens=30 * 52, Lq=0, d=128, block_q=128, block_k=128, n_cur_frames=0, q=0, frame_idx=0,
+                             frame_off_host=0, q_sb=0, q_sh=0, q_st=0, kv_sp=24 * 1560 * 128, kv_sh=1560 * 128,
+                             kv_st=128, H=24, grid_h=30, grid_w=52, bt=4, bh=8, bw=4)
+    assert L.li_slice_cache_bytes(ctypes.byref(p3)) == p3.n_pages * 24 * 4 * 13 * 128 * 4
+    assert L.li_pool_pages(ctypes.byref(p3), 0x50000, 0, 0x60000, None) == li.LI_OK                   # empty list: nothing to do
+    assert L.li_pool_pages(ctypes.byref(p3), 0x50000, 1, 0x60008, None) == li.LI_ERR_INVALID_ARG      # cache misaligned
+    p3.k_cache = 0
+    assert L.li_slice_cache_bytes(ctypes.byref(p3)) == 0
+
+
+def test_no_device_means_cuda_error_not_a_fallback(L):
+    """Without a CUDA device a compute call fails with LI_ERR_CUDA and li_last_cuda_error() names the runtime's code:
+    there is no CPU path to fall back to.  (Skipped where a GPU is present: the pointers are fake.)"""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    p, fo = make_problem()
+    tk = np.asarray([8], dtype=np.int32)
+    ws = L.li_workspace_bytes(ctypes.byref(p), 8)
+    assert L.li_block_select(ctypes.byref(p), tk.ctypes.data, 8, 0x60000, 0x70000, None, 0, 0x50000, ws, None) == li.LI_ERR_CUDA
+    assert L.li_last_cuda_error() != 0

@@ -250,10 +250,10 @@ def test_select_reuse_kbar_across_denoising_steps(P):
 
 
 @pytest.mark.parametrize("three_d", [False, True])
-def test_tail_wave_split_matches_oracle_and_unsplit_run(P, three_d, monkeypatch):
+def test_tail_wave_split_matches_oracle_and_unsplit_run(P, three_d):
     """Few query blocks with long tile lists: li_sparse_attn shares every query block between several CTAs (split of
     the last wave) and merges the partial results with a second launch.  The output must match the
-    oracle, and the unsplit run (LI_SPLIT_KV=0) up to fp32 rounding of the merge."""
+    oracle, and the unsplit run (li_problem.flags = LI_FLAG_NO_SPLIT) up to fp32 rounding of the merge."""
     import paper_2605_31158_b200 as li
     kw = dict(grid=(10, 20), block3d=(4, 8, 4)) if three_d else {}
     spec = W.spec_small(name="small-split", H=2, d=128, block=128, frame_tokens=200, n_cur_frames=3, n_pages=24,
@@ -261,13 +261,12 @@ def test_tail_wave_split_matches_oracle_and_unsplit_run(P, three_d, monkeypatch)
     prob = W.build(spec)
     li.lib().li_reset_launch_count()
     excused, mx, mean = P.full_parity(prob)
-    assert li.lib().li_launch_count() == 5, "3 select kernels + attention + merge expected (split not taken?)"
+    assert li.lib().li_launch_count() == 4, "2 select kernels + attention + merge expected (split not taken?)"
     ctx, buf = P.run_gpu(prob)
     o_split, lse_split = buf.o.float().cpu(), buf.lse.cpu()
-    monkeypatch.setenv("LI_SPLIT_KV", "0")
     li.lib().li_reset_launch_count()
-    ctx, buf = P.run_gpu(prob)
-    assert li.lib().li_launch_count() == 4
+    ctx, buf = P.run_gpu(prob, flags=li.LI_FLAG_NO_SPLIT)
+    assert li.lib().li_launch_count() == 3
     assert (buf.o.float().cpu() - o_split).abs().max() <= 4e-3       # one bf16 ulp of |o| <= 0.5
     assert (buf.lse.cpu() - lse_split).abs().max() <= 1e-5
     print(f"small-split: excused={excused} max-abs={mx:.3g} mean-abs={mean:.3g}")
@@ -293,7 +292,7 @@ def test_tail_wave_split_with_text_and_uneven_calls(P):
     li.lib().li_reset_launch_count()
     li.forward(ctx, prob.top_k, buf)
     torch.cuda.synchronize()
-    assert li.lib().li_launch_count() == 5, "split not taken"
+    assert li.lib().li_launch_count() == 4, "split not taken"
     osel, osc = P.oracle_select(prob)
     P.check_selection(prob, buf, osel, osc)
     gsel = [g_[0] for g_ in P.gpu_selection(prob, buf)]
@@ -306,7 +305,7 @@ def test_tail_wave_split_with_text_and_uneven_calls(P):
 
 
 def test_whole_step_is_cuda_graph_capturable(P):
-    """li_block_select + li_sparse_attn (4 launches with programmatic dependencies, here 5 with the split's merge) issue
+    """li_block_select + li_sparse_attn (3 launches with programmatic dependencies, here 4 with the split's merge) issue
     no synchronising call, so a step can be captured once and replayed; the replay must reproduce the eager outputs
     bit for bit, also after the inputs changed in place."""
     import paper_2605_31158_b200 as li
@@ -340,7 +339,7 @@ def test_tail_wave_split_other_tile_shapes(P, d, block):
     prob = W.build(spec)
     li.lib().li_reset_launch_count()
     excused, mx, mean = P.full_parity(prob)
-    assert li.lib().li_launch_count() == 5, "split not taken"
+    assert li.lib().li_launch_count() == 4, "split not taken"
     print(f"small-split d={d} block={block}: excused={excused} max-abs={mx:.3g} mean-abs={mean:.3g}")
 
 
@@ -361,3 +360,99 @@ def test_outputs_are_bitwise_repeatable(P):
         li.forward(ctx, prob.top_k, buf)
         torch.cuda.synchronize()
         assert torch.equal(buf.sel_idx, ref[0]) and torch.equal(buf.o, ref[1]) and torch.equal(buf.lse, ref[2]), it
+
+
+@pytest.mark.parametrize("T_f,block,d", [(8, 64, 64), (16, 128, 128), (24, 64, 128), (56, 128, 64)])
+def test_frames_shorter_than_half_a_block(P, T_f, block, d):
+    """frame_tokens < block/2: no tensor map with a half-tile box exists (AttnParams.has_box_full == 0), every K/V
+    half-tile is assembled from 8-row TMA boxes out of several pages, and the pool kernel looks a page up per row."""
+    spec = W.spec_small(name=f"small-shortframes-{T_f}-{block}", H=2, d=d, block=block, frame_tokens=T_f, n_cur_frames=11,
+                        n_pages=64, n_mem=(9,), n_win=(21,), density=Fraction(1, 2))
+    prob = W.build(spec)
+    assert T_f < block // 2 and prob.M(0) > 2 and prob.L_hist(0) % block != 0
+    excused, mx, mean = P.full_parity(prob)
+    print(f"{spec.name}: M={prob.M(0)} Nqb={prob.Nqb} excused={excused} max-abs={mx:.3g} mean-abs={mean:.3g}")
+
+
+def test_caller_built_unsorted_mask(P):
+    """li_sparse_attn takes a row of sel_idx as a SET (li.h: distinct values, any order).  A caller-built mask whose rows
+    are shuffled -- the partial history tail block M-1 first, in the middle or absent -- must give the oracle's result for
+    that set, and li_validate must accept it."""
+    import paper_2605_31158_b200 as li
+    spec = W.spec_small(name="small-unsorted", H=3, d=128, block=128, frame_tokens=200, n_cur_frames=2, n_pages=14,
+                        n_mem=(3,), n_win=(4,), density=Fraction(1, 2))
+    prob = W.build(spec)
+    M, k = prob.M(0), 6
+    assert prob.L_hist(0) % spec.block != 0 and M >= 8            # block M-1 is partial
+    rng = np.random.default_rng(31)
+    sel = np.full((1, spec.H, prob.Nqb, k), -1, np.int32)
+    cnt = np.zeros((1, spec.H, prob.Nqb), np.int32)
+    for h in range(spec.H):
+        for i in range(prob.Nqb):
+            c = int(rng.integers(1, k + 1))
+            row = rng.permutation(M - 1)[:c]
+            mode = (h + i) % 3                                    # 0: tail block first, 1: somewhere, 2: absent
+            if mode == 0:
+                row[0] = M - 1
+            elif mode == 1:
+                row[int(rng.integers(c))] = M - 1
+            sel[0, h, i, :c], cnt[0, h, i] = row, c
+    ctx = P.upload(prob)
+    buf = li.Buffers(ctx, k)
+    buf.sel_idx.copy_(torch.from_numpy(sel))
+    buf.sel_cnt.copy_(torch.from_numpy(cnt))
+    err = torch.full((4,), 7, dtype=torch.int32, device="cuda")
+    li.li_validate(ctx, err, buf.sel_idx, buf.sel_cnt, k)
+    li.li_sparse_attn(ctx, buf.sel_idx, buf.sel_cnt, k, buf.o, buf.lse, buf.workspace)
+    torch.cuda.synchronize()
+    assert err.tolist() == [0, 0, 0, 0]
+    o_ref, lse_ref = P.oracle_attn(prob, [sel[0]])
+    mx, mean = P.compare_output(buf.o, buf.lse, o_ref, lse_ref)
+    print(f"small-unsorted: max-abs {mx:.3g} mean-abs {mean:.3g}")
+
+
+def test_validate_reports_bad_device_inputs(P):
+    """li_validate (li.h): page ids outside the pool, sel_cnt > kmax, sel_idx outside [0, M_b), duplicates in a row --
+    each found on the device and reported through the caller's error word; a page id outside the pool is never
+    dereferenced by li_block_select (its rows count as zeros), so the call after a failed validation cannot fault."""
+    import paper_2605_31158_b200 as li
+    spec = W.spec_small(name="small-validate", H=2, d=128, block=128, frame_tokens=200, n_cur_frames=2, n_pages=16,
+                        n_mem=(2, 1), n_win=(3, 2), density=Fraction(1, 2), pages_per_call=8)
+    prob = W.build(spec)
+    ctx, buf = P.run_gpu(prob, want_scores=False)
+    err = torch.full((4,), 7, dtype=torch.int32, device="cuda")
+
+    def check(sel=None, cnt=None):
+        li.li_validate(ctx, err, sel, cnt, buf.kmax if sel is not None else 0)
+        torch.cuda.synchronize()
+        return err.tolist()
+
+    assert check() == [0, 0, 0, 0]
+    assert check(buf.sel_idx, buf.sel_cnt) == [0, 0, 0, 0]
+    # a page id outside the pool, in call 1's list
+    pos = int(prob.frame_off[1]) + 1
+    good = int(ctx.frame_idx[pos])
+    ctx.frame_idx[pos] = spec.n_pages + 5
+    assert check() == [li.LI_BAD_PAGE_ID, 2, pos, spec.n_pages + 5]
+    li.li_block_select(ctx, prob.top_k, buf.kmax, buf.sel_idx.clone(), buf.sel_cnt.clone(), buf.workspace)   # must not fault
+    torch.cuda.synchronize()
+    ctx.frame_idx[pos] = -1
+    assert check()[0] == li.LI_BAD_PAGE_ID
+    ctx.frame_idx[pos] = good
+    # selection lists
+    k0 = int(prob.top_k[0])
+    assert k0 >= 2
+    sel, cnt = buf.sel_idx.clone(), buf.sel_cnt.clone()
+    cnt[0, 1, 0] = buf.kmax + 1
+    assert check(sel, cnt) == [li.LI_BAD_SEL_CNT, 1, 1 * prob.Nqb + 0, buf.kmax + 1]
+    cnt.copy_(buf.sel_cnt)
+    sel[1, 0, 1, 0] = prob.M(1)
+    assert check(sel, cnt) == [li.LI_BAD_SEL_RANGE, 2, (0 * prob.Nqb + 1) * buf.kmax + 0, prob.M(1)]
+    sel.copy_(buf.sel_idx)
+    sel[0, 0, 0, 1] = sel[0, 0, 0, 0]
+    got = check(sel, cnt)
+    assert got[0] == li.LI_BAD_SEL_DUPLICATE and got[1] == 1 and got[2] in (0, 1) and got[3] == int(sel[0, 0, 0, 0])
+    sel[0, 0, 0, 0] = -3
+    assert check(sel, cnt)[0] == li.LI_BAD_SEL_RANGE
+    with pytest.raises(li.LiError):
+        li.li_validate(ctx, err, buf.sel_idx, None, buf.kmax)

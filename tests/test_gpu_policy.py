@@ -56,17 +56,61 @@ def test_policy_sequence_matches_oracle(env, dtype, n, nearest):
         assert r.D_bar == pytest.approx(Db_ref, rel=1e-5), "Eq. 2"
         assert ema.cpu().tolist() == [r.D_bar, 1.0]
         rounding = "nearest" if nearest else "floor"
-        # Eq. 3 decides an integer from a float: same precision (fp32) and operation order on both sides
-        assert r.L_t == PO.window_length(r.D_bar, kappa, L_max, rounding, np.float32)
+        # Eq. 3 decides an integer from a float.  The seeded inputs keep L_m kappa / (Dbar + kappa) at least 3.9e-3 away
+        # from every floor / round-half boundary (checked here), a thousand times the fp32-vs-fp64 difference of that
+        # quotient, so the INDEPENDENT fp64 decision of the oracle must be reproduced, unconditionally ...
         x = L_max * kappa / (Db_ref + kappa)
-        if abs(x - np.round(x * 2) / 2) > 1e-3:          # away from a rounding boundary: the fp64 decision as well
-            assert r.L_t == PO.window_length(Db_ref, kappa, L_max, rounding)
+        assert abs(x - np.round(x * 2) / 2) > 1e-3, "test input sits on a rounding boundary: pick another seed"
+        assert r.L_t == PO.window_length(Db_ref, kappa, L_max, rounding)
+        # ... and, as documented in li.h (operation order is part of the interface), the fp32 evaluation of the kernel's
+        # own Dbar as well
+        assert r.L_t == PO.window_length(r.D_bar, kappa, L_max, rounding, np.float32)
         keep = PO.keep_memory(s_pose, tau)
         assert bool(r.keep_memory) == keep, "Eq. 4"
         want = PO.reconstruct_frame_list(mem, win, cur, r.L_t, keep)
         assert r.n_frames == len(want) and r.n_hist_frames == len(want) - len(cur)
         np.testing.assert_array_equal(out[:r.n_frames], want)
         assert (out[r.n_frames:] == -7).all(), "entries past n_frames must stay untouched"
+
+
+@pytest.mark.parametrize("c,kappa,L_max,L_floor,L_nearest", [
+    (0.5, 0.25, 8, 4, 4),       # D = 1/4:  8 * 1/4 / (1/4 + 1/4)   = 4       exactly on an integer
+    (0.25, 0.25, 10, 8, 8),     # D = 1/16: 10 * 1/4 / (1/16 + 1/4) = 8       exactly on an integer
+    (0.5, 0.25, 5, 2, 2),       # D = 1/4:  5/4 / (1/2)             = 2.5     half-way: floor 2, nearest-even 2
+    (0.5, 0.25, 7, 3, 4),       # D = 1/4:  7/4 / (1/2)             = 3.5     half-way: floor 3, nearest-even 4
+    (1.0, 0.5, 3, 1, 1),        # D = 1:    3/2 / (3/2)             = 1       lower clip reached exactly
+    (0.0, 0.125, 6, 6, 6),      # D = 0:    6/8 / (1/8)             = 6 = L_m upper clip reached exactly
+    (2.0, 0.5, 16, 1, 2),       # D = 4:    8 / 4.5 = 1.777...      floor 1, nearest 2 (not a boundary)
+])
+def test_policy_window_length_on_exact_boundaries(env, c, kappa, L_max, L_floor, L_nearest):
+    """Eq. 3 on rounding boundaries whose answer is fixed by hand: z_{t-1} - z_{t-2} = c everywhere gives D_t = c^2 exactly
+    (c, c^2, kappa and L_m kappa are dyadic rationals, every fp32 and fp64 operation on them is exact), so
+    L_m kappa / (D + kappa) lands exactly on an integer or on a half: the expected L_t is the one written in the
+    parameter list, for both readings of the garbled bracket (DESIGN.md c18)."""
+    li, PO = env
+    n = 4096 + 24
+    z2 = torch.full((n,), 0.75).cuda()
+    z1 = torch.full((n,), 0.75 + c).cuda()
+    for nearest, want in ((False, L_floor), (True, L_nearest)):
+        ema = torch.zeros(2, dtype=torch.float32, device="cuda")
+        r, out = run_policy(li, z1, z2, ema, 1.0, kappa, L_max, [1.0], 0.5, [3], list(range(40, 60)), [7], nearest)
+        assert r.D_t == c * c and r.D_bar == c * c
+        assert r.L_t == want, (nearest, r.L_t, want)
+        assert r.n_frames == 1 + want + 1 and out[1:1 + want].tolist() == list(range(60 - want, 60))
+        assert PO.window_length(c * c, kappa, L_max, "nearest" if nearest else "floor") == want   # the oracle agrees by hand too
+
+
+def test_policy_ema_on_exact_values(env):
+    """Eq. 2 then Eq. 3 with dyadic values: D_1 = 1/4 initialises the EMA; D_2 = 1, alpha = 1/2 -> Dbar = 5/8 exactly;
+    kappa = 3/8, L_m = 8 -> 3 / 1 = 3 exactly."""
+    li, PO = env
+    n = 10007
+    ema = torch.zeros(2, dtype=torch.float32, device="cuda")
+    z2 = torch.zeros(n).cuda()
+    r, _ = run_policy(li, torch.full((n,), 0.5).cuda(), z2, ema, 0.5, 0.375, 8, [], 0.0, [], list(range(8)), [9])
+    assert (r.D_t, r.D_bar, r.L_t) == (0.25, 0.25, 4)                # 3 / (5/8) = 4.8 -> floor 4
+    r, _ = run_policy(li, torch.full((n,), 1.0).cuda(), z2, ema, 0.5, 0.375, 8, [], 0.0, [], list(range(8)), [9])
+    assert (r.D_t, r.D_bar, r.L_t) == (1.0, 0.625, 3)
 
 
 def test_policy_limits(env):
