@@ -31,11 +31,17 @@ import li_workloads as W
 
 METRIC = "sparse-attn effective TFLOP/s over attended blocks (select + attention, ms/call in ms_per_step)"
 UNIT = "TFLOP/s"
-# dram__bytes_read.sum + dram__bytes_write.sum of li_sparse_attn_kernel<128,128> per launch, from the
-# `ncu --set full` capture summarised in profiles/ (None until that capture exists for this workload).
-NCU_TRAFFIC_BYTES = {"mid": 400871936,     # profiles/r1d_mid_ncu_full_summary.txt: 366.19 MB read + 34.68 MB written
-                     "long": 1082519360,   # gpurun capture r1d (ncu --set full, same command with --config long): 1048.78 MB + 33.74 MB
-                     "mid3d": 408045056}   # profiles/r1b_mid3d_attn_ncu_summary.txt: 375.72 MB + 32.33 MB (split kernel)
+# roofline.traffic = dram__bytes_read.sum + dram__bytes_write.sum of the attention kernel per launch, taken from the
+# `ncu --set full` capture that profiles/traffic.json names for the workload (written from the extracted --page raw rows;
+# null when no capture of this workload is committed).
+def ncu_traffic(workload: str):
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        with open(path) as f:
+            e = json.load(f).get(workload)
+        return (int(e["dram_bytes"]), f"profiles/{e['source']}") if e else (None, None)
+    except (OSError, ValueError, KeyError):
+        return None, None
 
 
 def peaks():
@@ -469,11 +475,12 @@ def run_cuda(args):
             "select_gbs": sel_bytes / (float(sel_ms.mean()) * 1e-3) / 1e9,
             "frac_of_peak_burst": attn_tflops / pk["bf16_tflops"], "frac_of_peak_sustained": attn_tflops / pk["bf16_tflops_sustained"],
             "roofline": {"bound": "tensor", "achieved": attn_tflops, "peak": pk["bf16_tflops"], "unit": "TFLOP/s",
-                         "frac": attn_tflops / pk["bf16_tflops"], "traffic": NCU_TRAFFIC_BYTES.get(s.name),
+                         "frac": attn_tflops / pk["bf16_tflops"], "traffic": ncu_traffic(s.name)[0],
+                         "traffic_source": ncu_traffic(s.name)[1],
                          "kernel": "li_sparse_attn_kernel", "peak_source": pk["source"] + " burst bf16"},
             "roofline_select": {"bound": "hbm", "achieved": sel_bytes / (float(sel_ms.mean()) * 1e-3) / 1e9, "peak": pk["hbm_gbs"],
                                 "unit": "GB/s", "frac": sel_bytes / (float(sel_ms.mean()) * 1e-3) / 1e9 / pk["hbm_gbs"],
-                                "kernel": "li_pool_kernel + li_score_kernel + li_topk_kernel"},
+                                "kernel": "li_pool_kernel + li_score_topk_kernel"},
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "ms_per_step": e2e_ms / args.steps,
                     "head_groups": G,
@@ -500,7 +507,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--e2e-groups", type=int, default=4, help="head groups the end-to-end leg is pipelined over (1 = plain sequence)")
-    ap.add_argument("--config", default="mid", choices=["tiny", "mid", "long", "adaptive", "dense-equivalence", "mid3d", "long3d"])
+    ap.add_argument("--config", default="mid", choices=["tiny", "mid", "long", "adaptive", "dense-equivalence", "mid3d", "long3d", "mid3d448"])
     ap.add_argument("--ref-heads", type=int, default=24, help="heads in the oracle's bounded sample")
     ap.add_argument("--ref-tiles", type=int, default=None, help="query blocks per head in the oracle's sample (default all)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")

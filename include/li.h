@@ -71,10 +71,10 @@ typedef struct li_problem {
    * 128).  All five zero = 1-D blocks of block_k consecutive logical tokens.  Otherwise a frame is a grid_h x grid_w
    * row-major grid (frame_tokens == grid_h*grid_w, token = y*grid_w + x) and a region of n frames (history, chunk,
    * queries) is tiled by groups of bt consecutive frames x bh rows x bw columns; block index
-   * m = (tg*ceil(grid_h/bh) + hb)*ceil(grid_w/bw) + wb.  Border blocks (grid_h % bh != 0) and the last temporal group
-   * may be partial: padding never enters a mean nor the softmax, and is never stored.
-   * Supported: bt*bh*bw == block_q == block_k, bh*bw == 32, grid_w % bw == 0, Q contiguous over (B,H)
-   * (q_sb == H*q_sh). */
+   * m = (tg*ceil(grid_h/bh) + hb)*ceil(grid_w/bw) + wb.  Border blocks (grid_h % bh != 0, grid_w % bw != 0) and the last
+   * temporal group may be partial: padding never enters a mean nor the softmax, and is never stored (PAPER.md:148,
+   * :151).  Both of the paper's geometries run on the 30 x 52 grid: (4,8,4) and (4,4,8).
+   * Supported: bt*bh*bw == block_q == block_k, bh*bw == 32, Q contiguous over (B,H) (q_sb == H*q_sh). */
   int32_t grid_h, grid_w;
   int32_t bt, bh, bw;
   /* Text-conditioning tokens T of Eq. 11 (C_i = T U K^curr U S_i; "the model retains all

@@ -209,6 +209,14 @@ def spec_mid3d(H: int = 24) -> Spec:
                 n_mem=[4], n_win=[8], density=Fraction(1, 4), grid=(30, 52), block3d=(4, 8, 4))
 
 
+def spec_mid3d448(H: int = 24) -> Spec:
+    """`mid` with the paper's second block geometry, (4,4,8) (Matrix-Game-3.0), on the same 30 x 52 grid:
+    52 is not a multiple of 8, so every 7th column block is a half-width border block; 30 = 7*4 + 2 leaves a 2-row bottom
+    border."""
+    return Spec("mid3d448", 8008, H=H, d=128, frame_tokens=1560, n_cur_frames=4, block=128, n_pages=64,
+                n_mem=[4], n_win=[8], density=Fraction(1, 4), grid=(30, 52), block3d=(4, 4, 8))
+
+
 def spec_long3d(H: int = 24) -> Spec:
     """`long` (16 memory + 16 window frames, density 1/10, K offsets) with the paper's 3-D blocks: 416 history blocks."""
     return Spec("long3d", 7007, H=H, d=128, frame_tokens=1560, n_cur_frames=4, block=128, n_pages=128,
@@ -217,7 +225,8 @@ def spec_long3d(H: int = 24) -> Spec:
 
 def spec_by_name(name: str, H: Optional[int] = None) -> Spec:
     table = {"tiny": spec_tiny, "mid": spec_mid, "long": spec_long, "adaptive": spec_adaptive,
-             "dense-equivalence": spec_dense_equivalence, "mid3d": spec_mid3d, "long3d": spec_long3d}
+             "dense-equivalence": spec_dense_equivalence, "mid3d": spec_mid3d, "long3d": spec_long3d,
+             "mid3d448": spec_mid3d448}
     fn = table[name]
     if name == "tiny" or H is None:
         return fn()

@@ -132,7 +132,7 @@ int check_problem(const li_problem *p, Derived *dv, bool pages_only = false) {
     std::memset(&dv->tl, 0, sizeof(dv->tl));
     if (p->grid_h <= 0 || p->grid_w <= 0 || p->bt <= 0 || p->bh <= 0 || p->bw <= 0) return LI_ERR_UNSUPPORTED;
     if (p->grid_h * p->grid_w != p->frame_tokens) return LI_ERR_INVALID_ARG;
-    if (p->bt * p->bh * p->bw != p->block_k || p->bh * p->bw != 32 || p->grid_w % p->bw != 0) return LI_ERR_UNSUPPORTED;
+    if (p->bt * p->bh * p->bw != p->block_k || p->bh * p->bw != 32) return LI_ERR_UNSUPPORTED;
     dv->tl.gh = p->grid_h; dv->tl.gw = p->grid_w; dv->tl.bt = p->bt; dv->tl.bh = p->bh; dv->tl.bw = p->bw;
     dv->tl.Hb = (p->grid_h + p->bh - 1) / p->bh; dv->tl.Wb = (p->grid_w + p->bw - 1) / p->bw;
     for (dv->tl.bw_log2 = 0; (1 << dv->tl.bw_log2) < p->bw; ++dv->tl.bw_log2) {}
@@ -171,7 +171,7 @@ int check_problem(const li_problem *p, Derived *dv, bool pages_only = false) {
     if (p->grid_h <= 0 || p->grid_w <= 0 || p->bt <= 0 || p->bh <= 0 || p->bw <= 0) return LI_ERR_INVALID_ARG;
     if (p->grid_h * p->grid_w != p->frame_tokens) return LI_ERR_INVALID_ARG;
     if (p->Lq % p->frame_tokens != 0) return LI_ERR_INVALID_ARG;
-    if (p->bt * p->bh * p->bw != p->block_k || p->bh * p->bw != 32 || p->grid_w % p->bw != 0) return LI_ERR_UNSUPPORTED;
+    if (p->bt * p->bh * p->bw != p->block_k || p->bh * p->bw != 32) return LI_ERR_UNSUPPORTED;
     if (p->q_sb != (int64_t)p->H * p->q_sh && p->B > 1) return LI_ERR_UNSUPPORTED;
     dv->tl.gh = p->grid_h; dv->tl.gw = p->grid_w; dv->tl.bt = p->bt; dv->tl.bh = p->bh; dv->tl.bw = p->bw;
     dv->tl.Hb = (p->grid_h + p->bh - 1) / p->bh; dv->tl.Wb = (p->grid_w + p->bw - 1) / p->bw;

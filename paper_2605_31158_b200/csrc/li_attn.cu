@@ -83,8 +83,8 @@ __device__ __forceinline__ int64_t row_token(const AttnParams &p, int i, int row
   if (K3D) {
     const Tiling &tl = p.tl;
     const int per = tl.Hb * tl.Wb, tg = i / per, hb = (i - tg * per) / tl.Wb, wb = i - tg * per - hb * tl.Wb;
-    const int f = tg * tl.bt + (row >> 5), within = row & 31, y = hb * tl.bh + within / tl.bw;
-    return (row < BLK && f < p.Lq / p.T_f && y < tl.gh) ? (int64_t)f * p.T_f + y * tl.gw + wb * tl.bw + within % tl.bw : -1;
+    const int f = tg * tl.bt + (row >> 5), within = row & 31, y = hb * tl.bh + within / tl.bw, x = wb * tl.bw + within % tl.bw;
+    return (row < BLK && f < p.Lq / p.T_f && y < tl.gh && x < tl.gw) ? (int64_t)f * p.T_f + y * tl.gw + x : -1;
   }
   return row < min(BLK, p.Lq - i * BLK) ? (int64_t)i * BLK + row : -1;
 }
@@ -187,29 +187,28 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
   // 1-D: only two tiles can be partial: the last chunk block, and the history tail block M-1, wherever it sits in the
   // row's list (a row is a set: any order, li.h).  3-D: tiles of a region's last temporal group may hold fewer than bt
   // frames, border tiles fewer than bh grid rows.
-#ifdef LI_X_OLDTAIL
-  const int j_tail_hist = (cnt > 0 && sel_at(cnt - 1) == M - 1) ? n_tiles - 1 : -1;
-#else
   if (!k3d && tail_hist < BLK && cnt > 0) {            // CTA-uniform condition
     for (int t = threadIdx.x; t < cnt; t += blockDim.x)
       if (sel_at(t) == M - 1) *sTailPos = t;
     __syncthreads();
   }
   const int j_tail_hist = *sTailPos >= 0 ? Nt + Nc + *sTailPos : -1;
-#endif
   auto tile_valid = [&](int j) -> int {                // 1-D tiles (and text tiles in both modes): valid prefix
     if (TEXT && j < Nt) return j == Nt - 1 ? tail_text : BLK;
     return j == Nt + Nc - 1 ? tail_cur : (j == j_tail_hist ? tail_hist : BLK);
   };
   auto tile_blk = [&](int j) -> int { return j < Nt + Nc ? j - Nt : sel_at(j - Nt - Nc); };   // block index in its region
-  auto tile_info = [&](int j) -> int {                 // 3-D: (frames of tile j that exist) | (valid rows per slice) << 8
+  // 3-D: (frames of tile j that exist) | (valid grid columns if the block sticks out of the grid's right border, else 0) << 3
+  //       | (grid rows inside the grid * bw = valid prefix of a full-width slice) << 8
+  auto tile_info = [&](int j) -> int {
     int tg, hb, wb;
     split3(tile_blk(j), tg, hb, wb);
     const int nf = min(tl.bt, (j < Nt + Nc ? p.n_cur : n_hist) - tg * tl.bt);
-    return nf | (min(tl.bh, tl.gh - hb * tl.bh) * tl.bw) << 8;
+    const int vw = tl.gw - wb * tl.bw;
+    return nf | (vw < tl.bw ? vw : 0) << 3 | (min(tl.bh, tl.gh - hb * tl.bh) * tl.bw) << 8;
   };
   auto tile_info_cached = [&](int j) -> int { return j - Nt < kInfoCap ? (int)sInfo[j - Nt] : tile_info(j); };
-  auto tile_frames = [&](int j) -> int { return tile_info_cached(j) & 0xff; };
+  auto tile_frames = [&](int j) -> int { return tile_info_cached(j) & 7; };
   auto halves = [&](int j) -> int {                    // half-tiles of tile j with at least one valid key
     return (k3d && (!TEXT || j >= Nt)) ? (tile_frames(j) > SPH ? 2 : 1) : (tile_valid(j) > HALF ? 2 : 1);
   };
@@ -221,7 +220,7 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
       if (TEXT && j < Nt) { part += tile_valid(j) > HALF ? 2 : 1; continue; }
       const int info = tile_info(j);                   // integer divisions once per tile, not once per half-tile per role
       if (j - Nt < kInfoCap) sInfo[j - Nt] = (uint16_t)info;
-      part += (info & 0xff) > SPH ? 2 : 1;
+      part += (info & 7) > SPH ? 2 : 1;
     }
     if (part) atomicAdd(sT, part);
     __syncthreads();
@@ -428,14 +427,16 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
         }
       }
 
-#ifdef LI_X_OLDSOFTMAX
       for (int t = 0; t < Tn; ++t) {
-        // valid key columns of this half-tile, as a prefix length per 32-column slice (vs[s] rows of slice s are real,
-        // the rest is padding): 1-D blocks have one valid prefix; a 3-D slice is one frame's bh x bw patch, whose
-        // grid rows beyond grid_h (and whose frame, beyond the region) are padding
+        // valid key columns of this half-tile, as a prefix length per 32-column slice (vs[s] keys of slice s are real, the
+        // rest is padding): 1-D blocks have one valid prefix; a 3-D slice is one frame's bh x bw patch (key (y, x) in
+        // column y * bw + x), whose grid rows beyond grid_h (and whose frame, beyond the region) are padding; in a block
+        // over the grid's right border only vw of the bw columns exist
         int vs[SPH];
+        int vw = 0;
         if (k3d && (!TEXT || j >= Nt)) {
-          const int info = tile_info_cached(j), nf = info & 0xff, vrow = info >> 8;
+          const int info = tile_info_cached(j), nf = info & 7, vrow = info >> 8;
+          vw = (info >> 3) & 31;
 #pragma unroll
           for (int s_ = 0; s_ < SPH; ++s_) vs[s_] = (hh * SPH + s_ < nf) ? vrow : 0;
         } else {
@@ -443,9 +444,10 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
 #pragma unroll
           for (int s_ = 0; s_ < SPH; ++s_) vs[s_] = min(32, max(0, hv - 32 * s_));
         }
-        bool full = true;
+        bool rows_full = true;
 #pragma unroll
-        for (int s_ = 0; s_ < SPH; ++s_) full = full && vs[s_] == 32;
+        for (int s_ = 0; s_ < SPH; ++s_) rows_full = rows_full && vs[s_] == 32;
+        const bool full = rows_full && vw == 0;
         if (hh == 0 && halves(j) > 1) hh = 1;
         else { ++j; hh = 0; }
         const uint32_t s_addr = tmem + lane_base + (t & 1) * kSbCol;
@@ -456,7 +458,7 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
 #pragma unroll
         for (int c = 0; c < HALF / 32; ++c) tmem_ld32(s_addr + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&s[c * 32]));
         tc_wait_ld();
-        if (!full) {                                   // padded key columns -> -inf (warp-uniform branch)
+        if (!rows_full) {                              // padded key rows -> -inf (warp-uniform branch)
           bool same = k3d;                               // 3-D border tile: every slice has the same valid prefix,
 #pragma unroll
           for (int s_ = 1; s_ < SPH; ++s_) same = same && vs[s_] == vs[0];   // a multiple of bw rows
@@ -470,6 +472,11 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
             for (int c = 0; c < HALF; ++c) if ((c & 31) >= vs[c >> 5]) s[c] = 0xff800000u;
           }
         }
+        if (k3d && vw != 0) {                          // right-border block: grid columns x >= vw lie outside the grid
+          const int xm = tl.bw - 1;
+#pragma unroll
+          for (int c = 0; c < HALF; ++c) if ((c & xm) >= vw) s[c] = 0xff800000u;
+        }
         float mx0 = __uint_as_float(s[0]), mx1 = __uint_as_float(s[1]), mx2 = __uint_as_float(s[2]), mx3 = __uint_as_float(s[3]);
 #pragma unroll
         for (int c = 4; c < HALF; c += 4) {
@@ -478,11 +485,7 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
           mx2 = fmaxf(mx2, __uint_as_float(s[c + 2]));
           mx3 = fmaxf(mx3, __uint_as_float(s[c + 3]));
         }
-#ifdef LI_X_NOMAX
-        const float m_new = 4.0f;
-#else
         const float m_new = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * p.scale_log2;
-#endif
 
         // lazy rescale: the reference maximum only moves when the row maximum grew by more than 2^8
         bool need = false;
@@ -519,13 +522,8 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
           } else {
             float x0, x1;
             unpack2(x2, x0, x1);
-#ifdef LI_X_NOMUFU
-            p0 = fmaf(x0, 0.001f, 1.0f);
-            p1 = fmaf(x1, 0.001f, 1.0f);
-#else
             p0 = ex2_approx(x0);
             p1 = ex2_approx(x1);
-#endif
           }
           if (c & 1) sum_b = add2(sum_b, pack2(p0, p1));
           else sum_a = add2(sum_a, pack2(p0, p1));
@@ -544,174 +542,6 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
         if (lane == 0) mbar_arrive(bar(BAR_P_FULL + (t & 1)));
       }
 
-#else
-      // Valid key columns of half-tile (j, hh), as a prefix length per 32-column slice (vs[s] rows of slice s are real, the
-      // rest is padding): 1-D blocks have one valid prefix; a 3-D slice is one frame's bh x bw patch, whose grid rows
-      // beyond grid_h (and whose frame, beyond the region) are padding.  Returns whether every column is valid.
-      auto geometry = [&](int jj, int hv_, int (&vs)[SPH]) -> bool {
-        if (k3d && (!TEXT || jj >= Nt)) {
-          const int info = tile_info_cached(jj), nf = info & 0xff, vrow = info >> 8;
-#pragma unroll
-          for (int s_ = 0; s_ < SPH; ++s_) vs[s_] = (hv_ * SPH + s_ < nf) ? vrow : 0;
-        } else {
-          const int hv = min(HALF, tile_valid(jj) - hv_ * HALF);
-#pragma unroll
-          for (int s_ = 0; s_ < SPH; ++s_) vs[s_] = min(32, max(0, hv - 32 * s_));
-        }
-        bool full = true;
-#pragma unroll
-        for (int s_ = 0; s_ < SPH; ++s_) full = full && vs[s_] == 32;
-        return full;
-      };
-      uint32_t s[HALF];                                // one S row of the current half-tile (32-column chunks)
-      auto apply_mask = [&](const int (&vs)[SPH]) {    // padded key columns -> -inf (called under a warp-uniform branch)
-        bool same = k3d;                               // 3-D border tile: every slice has the same valid prefix,
-#pragma unroll
-        for (int s_ = 1; s_ < SPH; ++s_) same = same && vs[s_] == vs[0];   // a multiple of bw rows
-        if (same && (vs[0] & 7) == 0 && vs[0] > 0) {
-          // compile-time column positions: a few moves, no compares
-          if (vs[0] == 24) mask_slice_tail<24, HALF>(s);
-          else if (vs[0] == 16) mask_slice_tail<16, HALF>(s);
-          else mask_slice_tail<8, HALF>(s);
-        } else {
-#pragma unroll
-          for (int c = 0; c < HALF; ++c) if ((c & 31) >= vs[c >> 5]) s[c] = 0xff800000u;
-        }
-      };
-      auto load_chunk = [&](uint32_t s_addr, int ch) {
-        tmem_ld32(s_addr + ch * 32, *reinterpret_cast<uint32_t(*)[32]>(&s[ch * 32]));
-      };
-      auto chunk_max = [&](int ch) -> float {
-        float mx0 = __uint_as_float(s[ch * 32]), mx1 = __uint_as_float(s[ch * 32 + 1]), mx2 = __uint_as_float(s[ch * 32 + 2]),
-              mx3 = __uint_as_float(s[ch * 32 + 3]);
-#pragma unroll
-        for (int c = 4; c < 32; c += 4) {
-          mx0 = fmaxf(mx0, __uint_as_float(s[ch * 32 + c]));
-          mx1 = fmaxf(mx1, __uint_as_float(s[ch * 32 + c + 1]));
-          mx2 = fmaxf(mx2, __uint_as_float(s[ch * 32 + c + 2]));
-          mx3 = fmaxf(mx3, __uint_as_float(s[ch * 32 + c + 3]));
-        }
-        return fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
-      };
-      uint32_t pk[HALF / 2];
-      // P = exp2(s*scale - m_ref) for the 32 columns of chunk ch, bf16 pairs packed low = even column, row sums in fp32
-      auto chunk_exp = [&](int ch, float m_ref, uint64_t &sum_a, uint64_t &sum_b) {
-        const uint64_t sc2 = pack2(p.scale_log2, p.scale_log2), nm2 = pack2(-m_ref, -m_ref);
-#pragma unroll
-        for (int c = ch * 16; c < ch * 16 + 16; ++c) {
-          const uint64_t x2 = fma2(pack2(__uint_as_float(s[2 * c]), __uint_as_float(s[2 * c + 1])), sc2, nm2);
-          float p0, p1;
-          if ((c & 3) < kEmuOf4) {
-            exp2_emulated2(x2, p0, p1);
-          } else {
-            float x0, x1;
-            unpack2(x2, x0, x1);
-            p0 = ex2_approx(x0);
-            p1 = ex2_approx(x1);
-          }
-          if (c & 1) sum_b = add2(sum_b, pack2(p0, p1));
-          else sum_a = add2(sum_a, pack2(p0, p1));
-          pk[c] = pack_bf16x2(p0, p1);
-        }
-      };
-      constexpr int NCH = HALF / 32;
-
-      // Half-tile 0: its exact row maximum becomes the first reference maximum.  From then on the reference only moves
-      // when a row maximum exceeds it by more than 2^8 (lazy rescale), so the exponentials of half-tile t > 0 do not have
-      // to wait for that tile's own maximum: they start from the registers as soon as S(t) has landed, the maximum is
-      // taken alongside (FMNMX runs on the ALU pipe, the exponentials on the MUFU), and only if some row did outgrow the
-      // reference is the tile redone after the rescale (rare: the running maximum settles within the first tiles).
-      // S(t+1), computed by the tensor core while S(t) is being processed, is fetched into each 32-column chunk of the
-      // registers as soon as that chunk of S(t) has been consumed, so the TMEM load latency and the barrier round trip
-      // are off the warp's critical path as well.
-      int vs[SPH];
-      bool full = geometry(j, hh, vs);
-      mbar_wait(bar(BAR_S_FULL), 0);
-      tc_fence_after();
-#pragma unroll
-      for (int ch = 0; ch < NCH; ++ch) load_chunk(tmem + lane_base, ch);
-      tc_wait_ld();
-      if (!full) apply_mask(vs);
-      {
-        float mx = chunk_max(0);
-#pragma unroll
-        for (int ch = 1; ch < NCH; ++ch) mx = fmaxf(mx, chunk_max(ch));
-        m_used = mx * p.scale_log2;
-      }
-      bool landed = true;                              // S(t) is in the registers, masked
-      for (int t = 0; t < Tn; ++t) {
-        const uint32_t s_addr = tmem + lane_base + (t & 1) * kSbCol, s_next = tmem + lane_base + ((t + 1) & 1) * kSbCol;
-        const bool has_next = t + 1 < Tn;
-        if (t > 0) full = geometry(j, hh, vs);
-        if (hh == 0 && halves(j) > 1) hh = 1;
-        else { ++j; hh = 0; }
-        if (!landed) {                                 // S(t) was not ready when the previous tile tried to prefetch it
-          mbar_wait(bar(BAR_S_FULL + (t & 1)), (t >> 1) & 1);
-          tc_fence_after();
-#pragma unroll
-          for (int ch = 0; ch < NCH; ++ch) load_chunk(s_addr, ch);
-        }
-        if (t > 0) {
-          tc_wait_ld();
-          if (!full) apply_mask(vs);
-        }
-        // is S(t+1) complete already?  (one uniform poll; the answer only decides WHEN it is fetched)
-        const bool pre = has_next && __all_sync(0xffffffffu, mbar_try_wait(bar(BAR_S_FULL + ((t + 1) & 1)), ((t + 1) >> 1) & 1));
-        if (pre) tc_fence_after();
-        uint64_t sum_a = pack2(0.f, 0.f), sum_b = pack2(0.f, 0.f);
-        float mx = __int_as_float(0xff800000);
-#pragma unroll
-        for (int ch = 0; ch < NCH; ++ch) {
-          mx = fmaxf(mx, chunk_max(ch));
-          chunk_exp(ch, m_used, sum_a, sum_b);
-          if (pre) load_chunk(s_next, ch);             // this chunk's registers are free: fetch S(t+1) into them
-        }
-        landed = pre;
-        const float m_new = mx * p.scale_log2;
-        const bool need = m_new > m_used + kRescaleThreshold;
-        if (__ballot_sync(0xffffffffu, need)) {
-          // Some row outgrew its reference maximum: move it, rescale O, redo this tile's exponentials.
-          // O is being accumulated by PV(t-1): wait for it (PV(t-2) is known complete, so the parity is unambiguous)
-          if (pre) tc_wait_ld();                       // the prefetched S(t+1) is dropped and fetched again below
-          mbar_wait(bar(BAR_PV_DONE), (t - 1) & 1);
-          tc_fence_after();
-          const float f = need ? ex2_approx(m_used - m_new) : 1.0f;
-          if (need) { m_used = m_new; l *= f; }
-#pragma unroll 1
-          for (int c = 0; c < D / 32; ++c) {
-            uint32_t o[32];
-            tmem_ld32(tmem + lane_base + kOCol + c * 32, o);
-            tc_wait_ld();
-#pragma unroll
-            for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * f);
-            tmem_st32(tmem + lane_base + kOCol + c * 32, o);
-          }
-#pragma unroll
-          for (int ch = 0; ch < NCH; ++ch) load_chunk(s_addr, ch);
-          tc_wait_ld();
-          if (!full) apply_mask(vs);
-          sum_a = pack2(0.f, 0.f);
-          sum_b = pack2(0.f, 0.f);
-#pragma unroll
-          for (int ch = 0; ch < NCH; ++ch) chunk_exp(ch, m_used, sum_a, sum_b);
-          if (pre) {
-#pragma unroll
-            for (int ch = 0; ch < NCH; ++ch) load_chunk(s_next, ch);
-          }
-        }
-        {
-          float a0, a1;
-          unpack2(add2(sum_a, sum_b), a0, a1);
-          l += a0 + a1;
-        }
-        if constexpr (HALF == 64) tmem_st32(s_addr, *reinterpret_cast<uint32_t(*)[32]>(&pk[0]));
-        else tmem_st16(s_addr, pk);
-        tc_wait_st();
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(bar(BAR_P_FULL + (t & 1)));
-      }
-#endif
 
       mbar_wait(bar(BAR_O_FULL), 0);
       tc_fence_after();

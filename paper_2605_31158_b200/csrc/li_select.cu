@@ -156,84 +156,128 @@ __device__ __forceinline__ uint32_t order_key(float s) {
 }
 
 // ----------------------------------------------------------------------------- fused scores + Top_k (Eq. 10), M <= 512
-// One CTA = 8 consecutive query-block rows of one (call, head); grid = (ceil(Nqb / 8), B*H), 8 warps.
-// Phase 1 (scores): warp w = (row half rh = w / 4, channel quarter cq = w % 4) accumulates, for its 4 rows, the partial
-//   dot products over channels [cq*D/4, (cq+1)*D/4): lane = historical block m = lane + 32 x, x < NX, i.e. 4 * NX
-//   independent fp32 FMA chains per lane; kbar is channel-major, so for a fixed channel the 32 lanes read one 128-byte
-//   line and every loaded value feeds 4 FMAs; the pooled query rows are broadcast from shared memory.  The loads of the
-//   next channel pair are issued before the FMAs of the current one.  Partials -> shared memory [cq][row][Mp].
-// Phase 2 (Top_k): warp w owns row w: the 4 partial sums of a score are added in a fixed order (cq = 0..3), the scores
-//   stay in registers as order-preserving keys, the k-th largest is found by an MSB-first radix select (32 counting
-//   passes with redux.sync), and one ordered pass emits, ascending, every block above the threshold plus the
-//   lowest-index blocks equal to it.
-constexpr int kSelRows = 8;
+// One CTA = up to 16 consecutive query-block rows of one (call, head); grid = (ceil(Nqb / rows), B*H), 16 warps.
+// The head's pooled keys kbar[bh] (channel-major [D][Mp], contiguous) are streamed into shared memory by bulk async
+// copies (cp.async.bulk + mbarrier), one per channel quarter, all issued up front (fewer when four do not fit; the
+// others follow into the slots read first): no load latency is paid per FMA and no register holds data in flight.
+// Phase 1 (scores): warp w = (32-block group g = w mod nxp, channel part cp = w / nxp) holds ALL 16 rows against the 32
+//   blocks m = 32 g + lane (nxp = Mp / 32 groups): per channel one conflict-free LDS of kbar, four broadcast LDS.128 of the 16 pooled query
+//   values and 8 packed FMAs (fma.rn.f32x2: two rows per instruction).  The 16 / nxp channel parts take interleaved
+//   channels; their partial sums go to shared memory [part][row][Mp].
+// Phase 2 (Top_k): warp w owns row w: a score is the sum of its parts in a fixed order; the scores stay in registers as
+//   order-preserving keys, the k-th largest is found by an MSB-first radix select (32 counting passes with
+//   redux.sync), and one ordered pass emits, ascending, every block above the threshold plus the lowest-index blocks
+//   equal to it.
+constexpr int kSelWarps = 16;
+constexpr int kSelRowsMax = 16;
+constexpr int kSelPartFloats = kSelRowsMax * 16 * 32;      // [parts][16 rows][Mp] with parts * Mp <= 16 * 32
+__host__ __device__ inline size_t sel_smem_bytes(int D, int Mp, int n_slots) {
+  return 128 + (size_t)(D * kSelRowsMax + kSelPartFloats + n_slots * (D / 4) * Mp) * sizeof(float);
+}
+// pooled query value (channel c, row r) lives at float c*16 + 4*((r/4) ^ (c & 3)) + r%4: a warp reads 4 consecutive rows
+// with one broadcast LDS.128 (the XOR permutes whole row quads) and the channel-major staging stores of consecutive
+// channels spread over the banks
+__device__ __forceinline__ int sq_index(int c, int r) { return c * kSelRowsMax + ((((r >> 2) ^ (c & 3)) << 2) | (r & 3)); }
+
 template <int D, int NX>
-__global__ void __launch_bounds__(kSelRows * 32) li_score_topk_kernel(const SelectParams p, const BatchMeta meta) {
-  extern __shared__ __align__(16) float sel_smem[];
-  constexpr int DW = D / 4;                                // channels per warp
-  float *sq = sel_smem;                                    // [8 rows][D]
-  float *part = sel_smem + kSelRows * D;                   // [4 quarters][8 rows][Mp]
+__global__ void __launch_bounds__(kSelWarps * 32) li_score_topk_kernel(const SelectParams p, const BatchMeta meta,
+                                                                        const int rows_per_cta, const int n_slots) {
+  extern __shared__ __align__(128) uint8_t sel_smem[];
+  constexpr int DW = D / 4;
+  float *sqT = reinterpret_cast<float *>(sel_smem + 128);  // [D][16], see sq_index
+  float *part = sqT + D * kSelRowsMax;                     // [parts][16][Mp]: partial dot products
+  float *ring = part + kSelPartFloats;                     // [n_slots][DW][Mp]: channel quarters of kbar[bh]
+  const uint32_t bar0 = smem_u32(sel_smem);                // 4 mbarriers, one per channel quarter (each used once)
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int bh = blockIdx.y, b = bh / p.H;
-  const int i0 = blockIdx.x * kSelRows;
+  const int i0 = blockIdx.x * rows_per_cta, R = min(rows_per_cta, p.Nqb - i0);
   const int n_hist = meta.frame_off[b + 1] - meta.frame_off[b] - p.n_cur;
   const int M = p.tl.num_blocks(n_hist, p.T_f, p.blk);
   const int k = min(meta.top_k[b], M);
-  const int nx = (M + 31) >> 5;                            // 32-block groups that exist (CTA-uniform)
+  const int nx = (M + 31) >> 5;                            // 32-block groups that exist (CTA-uniform), <= 16
+  const int nxp = p.Mp >> 5;                               // groups the row pitch holds (>= nx, batch-uniform), <= 16
+  const int parts = kSelWarps / nxp;                       // channel parts (warps per group); parts * Mp <= 16 * 32
+  const bool scoring = M > 0 && (k > 0 || p.scores != nullptr);   // CTA-uniform
+  const uint32_t quarter_bytes = (uint32_t)(DW * p.Mp * sizeof(float));
+  const float *ksrc = p.kbar + (int64_t)bh * D * p.Mp;
+  auto copy_quarter = [&](int q) {                         // one elected thread
+    const uint32_t mb = bar0 + 8u * q, dst = smem_u32(ring) + (uint32_t)(q % n_slots) * quarter_bytes;
+    mbar_arrive_expect_tx(mb, quarter_bytes);
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(ksrc + (size_t)q * DW * p.Mp), "r"(quarter_bytes), "r"(mb) : "memory");
+  };
+  if (threadIdx.x == 0) {
+    for (int q = 0; q < 4; ++q) mbar_init(bar0 + 8u * q, 1);
+    mbar_fence_init();
+    fence_proxy_async();
+  }
   pdl_launch_dependents();
   pdl_wait();                                              // qbar / kbar come from li_pool_kernel
-
-  if (M > 0 && (k > 0 || p.scores != nullptr)) {
-    for (int t = threadIdx.x; t < kSelRows * D / 4; t += kSelRows * 32) {
-      const int g = t / (D / 4);
-      reinterpret_cast<float4 *>(sq)[t] =
-          (i0 + g < p.Nqb) ? __ldg(reinterpret_cast<const float4 *>(p.qbar + ((int64_t)bh * p.Nqb + i0) * D) + t)
-                           : make_float4(0.f, 0.f, 0.f, 0.f);
+  if (scoring) {
+    if (threadIdx.x == 0)
+      for (int q = 0; q < n_slots; ++q) copy_quarter(q);
+    for (int t = threadIdx.x; t < kSelRowsMax * D; t += kSelWarps * 32) {
+      const int r = t / D, c = t - r * D;
+      sqT[sq_index(c, r)] = r < R ? __ldg(p.qbar + ((int64_t)bh * p.Nqb + i0 + r) * D + c) : 0.f;
     }
-    const int rh = warp >> 2, cq = warp & 3;
-    const float *kT = p.kbar + ((int64_t)bh * D + cq * DW) * p.Mp + lane;   // lanes past M read the row's padding; dropped
-    float acc[4][NX];
+    __syncthreads();                                       // barriers initialised, query values staged
+    const int g = warp % nxp, cp = warp / nxp;             // idle: cp >= parts (16 is not a multiple of nxp), g >= nx (short call)
+    uint64_t acc[kSelRowsMax / 2];                         // acc[rp] = (row 2 rp, row 2 rp + 1) against block 32 g + lane
 #pragma unroll
-    for (int r = 0; r < 4; ++r)
+    for (int rp = 0; rp < kSelRowsMax / 2; ++rp) acc[rp] = 0ull;
+    for (int q = 0; q < 4; ++q) {
+      mbar_wait(bar0 + 8u * q, 0);
+      if (cp < parts && g < nx) {
+        const float *kq = ring + (size_t)(q % n_slots) * DW * p.Mp + 32 * g + lane;
+        const float *qq = sqT + (size_t)q * DW * kSelRowsMax;
+        // this part's channels of the quarter: c = cp, cp + parts, ...; unrolled by 4 with the loads up front
+        int c = cp;
+        for (; c + 3 * parts < DW; c += 4 * parts) {
+          float kv[4];
 #pragma unroll
-      for (int x = 0; x < NX; ++x) acc[r][x] = 0.f;
-    float kv[2][2][NX];                                    // [buffer][channel of the pair][group]
-    auto load_pair = [&](int buf, int c) {
+          for (int u = 0; u < 4; ++u) kv[u] = kq[(size_t)(c + u * parts) * p.Mp];
 #pragma unroll
-      for (int cc = 0; cc < 2; ++cc)
+          for (int u = 0; u < 4; ++u) {
+            const int cc = c + u * parts;
+            const uint64_t kk = pack2(kv[u], kv[u]);
 #pragma unroll
-        for (int x = 0; x < NX; ++x) kv[buf][cc][x] = x < nx ? __ldg(kT + (int64_t)(c + cc) * p.Mp + 32 * x) : 0.f;
-    };
-    auto fma_pair = [&](int buf, int c) {
-#pragma unroll
-      for (int cc = 0; cc < 2; ++cc)
-#pragma unroll
-        for (int r = 0; r < 4; ++r) {
-          const float qc = sq[(rh * 4 + r) * D + cq * DW + c + cc];
-#pragma unroll
-          for (int x = 0; x < NX; ++x) acc[r][x] = fmaf(qc, kv[buf][cc][x], acc[r][x]);
+            for (int rq = 0; rq < 4; ++rq) {
+              const float4 q4 = *reinterpret_cast<const float4 *>(qq + cc * kSelRowsMax + ((rq ^ (cc & 3)) << 2));
+              acc[2 * rq] = fma2(pack2(q4.x, q4.y), kk, acc[2 * rq]);
+              acc[2 * rq + 1] = fma2(pack2(q4.z, q4.w), kk, acc[2 * rq + 1]);
+            }
+          }
         }
-    };
-    load_pair(0, 0);
-    __syncthreads();                                       // sq staged
-#pragma unroll 1
-    for (int c = 0; c < DW; c += 4) {
-      load_pair(1, c + 2);
-      fma_pair(0, c);
-      if (c + 4 < DW) load_pair(0, c + 4);
-      fma_pair(1, c + 2);
+        for (; c < DW; c += parts) {
+          const float kv = kq[(size_t)c * p.Mp];
+          const uint64_t kk = pack2(kv, kv);
+#pragma unroll
+          for (int rq = 0; rq < 4; ++rq) {
+            const float4 q4 = *reinterpret_cast<const float4 *>(qq + c * kSelRowsMax + ((rq ^ (c & 3)) << 2));
+            acc[2 * rq] = fma2(pack2(q4.x, q4.y), kk, acc[2 * rq]);
+            acc[2 * rq + 1] = fma2(pack2(q4.z, q4.w), kk, acc[2 * rq + 1]);
+          }
+        }
+      }
+      if (q + n_slots < 4) {                               // the ring is shorter than the head: refill the slot just read
+        __syncthreads();
+        if (threadIdx.x == 0) copy_quarter(q + n_slots);
+      }
     }
+    if (cp < parts && g < nx) {
 #pragma unroll
-    for (int r = 0; r < 4; ++r)
-#pragma unroll
-      for (int x = 0; x < NX; ++x)
-        if (x < nx) part[((size_t)cq * kSelRows + rh * 4 + r) * p.Mp + lane + 32 * x] = acc[r][x];
+      for (int rp = 0; rp < kSelRowsMax / 2; ++rp) {
+        float s0, s1;
+        unpack2(acc[rp], s0, s1);
+        part[((size_t)cp * kSelRowsMax + 2 * rp) * p.Mp + 32 * g + lane] = s0;
+        part[((size_t)cp * kSelRowsMax + 2 * rp + 1) * p.Mp + 32 * g + lane] = s1;
+      }
+    }
   }
   __syncthreads();
 
-  const int i = i0 + warp;
-  if (i >= p.Nqb) return;                                  // whole warp; no CTA-wide barrier below
-  const int64_t row = (int64_t)bh * p.Nqb + i;
+  if (warp >= R) return;                                   // whole warp; no CTA-wide barrier below
+  const int64_t row = (int64_t)bh * p.Nqb + i0 + warp;
   int32_t *out = p.sel_idx + row * p.kmax;
   if (lane == 0) p.sel_cnt[row] = k;
   uint32_t kr[NX];
@@ -241,13 +285,12 @@ __global__ void __launch_bounds__(kSelRows * 32) li_score_topk_kernel(const Sele
   for (int x = 0; x < NX; ++x) {
     const int m = lane + 32 * x;
     kr[x] = 0u;                                            // absent blocks: key 0, below every real key
-    if (m < M && (k > 0 || p.scores != nullptr)) {
-      const float *pr = part + (size_t)warp * p.Mp + m;
-      const size_t qs = (size_t)kSelRows * p.Mp;
-      const float dot = ((pr[0] + pr[qs]) + pr[2 * qs]) + pr[3 * qs];
-      const float sc = dot * p.inv_sqrt_d + 0.0f;          // -0 -> +0 so that equal scores have equal keys
-      kr[x] = order_key(sc);
-      if (p.scores != nullptr) p.scores[row * p.score_pitch + m] = sc;
+    if (m < M && scoring) {
+      float dot = part[(size_t)warp * p.Mp + m];
+      for (int pp = 1; pp < parts; ++pp) dot += part[((size_t)pp * kSelRowsMax + warp) * p.Mp + m];   // fixed order
+      const float sv = dot * p.inv_sqrt_d + 0.0f;          // -0 -> +0 so that equal scores have equal keys
+      kr[x] = order_key(sv);
+      if (p.scores != nullptr) p.scores[row * p.score_pitch + m] = sv;
     }
   }
   if (k > 0) {
@@ -435,31 +478,36 @@ int launch_pool_pages(const SelectParams &sp, const int32_t *pages, int n_list, 
   return (int)cudaGetLastError();
 }
 
+constexpr size_t kSelSmemMax = 227 * 1024;
 template <int D, int NX>
 static cudaError_t launch_score_topk_nx(cudaLaunchConfig_t &cfg, const SelectParams &sp, const BatchMeta &meta) {
-  // shared memory: 8 pooled query rows + the partial sums [4][8][Mp]; above 48 KB the limit is raised once per device
-  cfg.dynamicSmemBytes = (size_t)(kSelRows * D + 4 * kSelRows * sp.Mp) * sizeof(float);
-  if (cfg.dynamicSmemBytes > 48 * 1024) {
+  // rows per CTA: the fewest CTAs per head whose rows fit 16 warps, rows spread evenly (49 rows -> 4 CTAs of 13, 13, 13, 10)
+  const int groups = (sp.Nqb + kSelRowsMax - 1) / kSelRowsMax, rows = (sp.Nqb + groups - 1) / groups;
+  int n_slots = 4;                                         // channel quarters of kbar[bh] resident at once (2 always fit)
+  while (n_slots > 1 && sel_smem_bytes(D, sp.Mp, n_slots) > kSelSmemMax) --n_slots;
+  cfg.gridDim = dim3(groups, sp.B * sp.H);
+  cfg.blockDim = dim3(kSelWarps * 32);
+  cfg.dynamicSmemBytes = sel_smem_bytes(D, sp.Mp, n_slots);
+  if (cfg.dynamicSmemBytes > 48 * 1024) {                  // above 48 KB the limit is raised once per device
     static std::atomic<uint64_t> attr_done{0};
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
     const uint64_t dev_bit = 1ull << (dev & 63);
     if (!(attr_done.load(std::memory_order_acquire) & dev_bit)) {
-      e = cudaFuncSetAttribute(li_score_topk_kernel<D, NX>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                               (kSelRows * D + 4 * kSelRows * 512) * (int)sizeof(float));
+      e = cudaFuncSetAttribute(li_score_topk_kernel<D, NX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSelSmemMax);
       if (e != cudaSuccess) return e;
       attr_done.fetch_or(dev_bit, std::memory_order_release);
     }
   }
-  return cudaLaunchKernelEx(&cfg, li_score_topk_kernel<D, NX>, sp, meta);
+  return cudaLaunchKernelEx(&cfg, li_score_topk_kernel<D, NX>, sp, meta, rows, n_slots);
 }
 template <int D>
 static cudaError_t launch_score_topk(cudaLaunchConfig_t &cfg, const SelectParams &sp, const BatchMeta &meta) {
   if (sp.Mmax <= 128) return launch_score_topk_nx<D, 4>(cfg, sp, meta);
   if (sp.Mmax <= 192) return launch_score_topk_nx<D, 6>(cfg, sp, meta);
   if (sp.Mmax <= 256) return launch_score_topk_nx<D, 8>(cfg, sp, meta);
-  if (sp.Mmax <= 384) return launch_score_topk_nx<D, 12>(cfg, sp, meta);
+  if (sp.Mmax <= 416) return launch_score_topk_nx<D, 13>(cfg, sp, meta);
   return launch_score_topk_nx<D, 16>(cfg, sp, meta);
 }
 
@@ -485,8 +533,6 @@ int launch_select(const SelectParams &sp, const BatchMeta &meta, cudaStream_t st
   cfg.attrs = attr;
   cfg.numAttrs = 1;
   if (sp.Mmax <= 512) {
-    cfg.gridDim = dim3((sp.Nqb + kSelRows - 1) / kSelRows, sp.B * sp.H);
-    cfg.blockDim = dim3(kSelRows * 32);
     cudaError_t e = sp.d == 128 ? launch_score_topk<128>(cfg, sp, meta) : launch_score_topk<64>(cfg, sp, meta);
     if (e != cudaSuccess) return (int)e;
     if (n_launches) *n_launches += 1;

@@ -118,7 +118,9 @@ def test_3d_tiling_validation(L):
     assert ws == (24 * 52 * 128 * 4 + 24 * 128 * 64 * 4 + 24 * 52 * 52 * 4 + (256 - (24 * 52 * 52 * 4) % 256) % 256
                   + 320 * 128 * (128 * 4 + 8))
     for bad, code in ((dict(bw=8), li.LI_ERR_UNSUPPORTED),            # 4*8*8 != 128
-                      (dict(bh=4, bw=8), li.LI_ERR_UNSUPPORTED),       # 52 % 8 != 0
+                      (dict(bh=4, bw=8), li.LI_OK),                    # (4,4,8) on a 52-wide grid: partial right border
+                      (dict(bh=16, bw=2), li.LI_OK),                   # any bh*bw == 32
+                      (dict(bh=8, bw=8, bt=2), li.LI_ERR_UNSUPPORTED), # bh*bw != 32
                       (dict(grid_w=50), li.LI_ERR_INVALID_ARG),        # grid_h*grid_w != frame_tokens
                       (dict(bt=0), li.LI_ERR_INVALID_ARG),             # partially specified
                       (dict(bt=2, block_q=64, block_k=64), li.LI_OK)): # (2,8,4) = 64-token blocks

@@ -26,7 +26,9 @@ def small3d(name, grid, block3d, n_cur, n_mem, n_win, H=2, d=128, density=Fracti
 @pytest.mark.parametrize("grid,block3d,n_cur,n_hist", [((30, 52), (4, 8, 4), 4, (2, 4)),     # paper geometry, partial rows
                                                         ((10, 16), (4, 4, 8), 4, (3, 3)),     # Matrix-Game block shape
                                                         ((12, 8), (2, 8, 4), 2, (2, 3)),      # 64-token blocks, partial group
-                                                        ((6, 8), (4, 8, 4), 3, (1, 4))])      # grid lower than a block, partial groups
+                                                        ((6, 8), (4, 8, 4), 3, (1, 4)),       # grid lower than a block, partial groups
+                                                        ((30, 52), (4, 4, 8), 4, (2, 4)),     # Matrix-Game shape on the 52-wide grid
+                                                        ((9, 24), (4, 2, 16), 2, (3, 2))])    # 16-wide blocks: 8 of 16 columns at the border
 def test_select_3d(P, grid, block3d, n_cur, n_hist):
     spec = small3d(f"s3d-{grid}-{block3d}", grid, block3d, n_cur, (n_hist[0],), (n_hist[1],))
     prob = W.build(spec)
@@ -37,7 +39,10 @@ def test_select_3d(P, grid, block3d, n_cur, n_hist):
 @pytest.mark.parametrize("grid,block3d,n_cur,n_hist,d", [((30, 52), (4, 8, 4), 4, (2, 4), 128),   # paper geometry: rows 24..29 partial
                                                           ((10, 16), (4, 4, 8), 4, (3, 3), 128),   # (4,4,8), partial group (6 frames)
                                                           ((12, 8), (2, 8, 4), 2, (2, 3), 64),     # 64-token blocks, d=64
-                                                          ((6, 8), (4, 8, 4), 3, (1, 4), 128)])    # partial chunk group (3 of 4 frames)
+                                                          ((6, 8), (4, 8, 4), 3, (1, 4), 128),     # partial chunk group (3 of 4 frames)
+                                                          ((30, 52), (4, 4, 8), 4, (2, 4), 128),   # (4,4,8) on 30 x 52: right AND bottom borders
+                                                          ((10, 12), (2, 4, 8), 2, (2, 3), 64),    # 64-token blocks, 4-of-8-column border
+                                                          ((9, 24), (4, 2, 16), 2, (3, 2), 128)])  # 16-wide blocks, 1-row bottom border
 def test_full_parity_3d(P, grid, block3d, n_cur, n_hist, d):
     """li_block_select + li_sparse_attn with 3-D blocks, element by element against the oracle: 5-D TMA boxes, zero
     filled grid rows / missing frames masked out, outputs scattered back to linear token order."""

@@ -124,6 +124,18 @@ def test_mid3d_full_size_mask_and_stratified_attention(P):
     assert n_border >= 24 and mask.sum() == (len(tiles) - n_border) * 128 + n_border * 96
 
 
+def test_mid3d448_full_size_mask_and_stratified_attention(P):
+    """`mid` shapes with the paper's second geometry, (4,4,8) blocks, on the 30 x 52 grid: 8 x 7 blocks per
+    temporal group; every 7th column block holds 4 of 8 columns, the bottom row of blocks 2 of 4 rows (128 / 64 / 32
+    tokens).  56 query blocks x 24 heads = 1344 CTAs = 4.54 waves (no split)."""
+    prob = W.build(W.spec_by_name("mid3d448"))
+    assert prob.M(0) == 168 and prob.Nqb == 56 and int(prob.top_k[0]) == 42
+    tiles = stratified_tiles(prob)
+    ctx, buf, mask = run_and_check(P, prob, tiles)
+    sizes = prob.block_sizes(4)
+    assert mask.sum() == sum(int(sizes[t[2]]) for t in tiles)
+
+
 def test_long3d_full_size_mask_and_stratified_attention(P):
     """`long` shapes (32 history frames, K offsets per page and head, density 1/10) with 3-D (4,8,4) blocks: 416 history
     blocks, k = 41; 1248 query blocks = 4.22 waves, so the tail-wave split runs at full size."""
