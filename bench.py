@@ -218,7 +218,22 @@ def run_cuda(args):
     kc = prob.k_cache.to(dev)
     vc = prob.v_cache.to(dev)
     fi = torch.from_numpy(prob.frame_idx).to(dev)
-    ctx = li.Context(q, kc, vc, fi, prob.frame_off, s.n_cur_frames, s.block, grid=s.grid, block3d=s.block3d)
+    fp8 = args.kv == "fp8"
+    if fp8:
+        # FP8 (E4M3) K/V pages: one scale per head = max |value| of the pool / 448; the pool is quantised
+        # once here (untimed), the chunk's pages again inside every end-to-end step (quantise-on-write)
+        k_scale = (kc.float().abs().amax(dim=(0, 2, 3)) / 448.0).contiguous()
+        v_scale = (vc.float().abs().amax(dim=(0, 2, 3)) / 448.0).contiguous()
+        k8, v8 = torch.empty(kc.shape, dtype=torch.uint8, device=dev), torch.empty(vc.shape, dtype=torch.uint8, device=dev)
+        ctx = li.Context(q, k8, v8, fi, prob.frame_off, s.n_cur_frames, s.block, grid=s.grid, block3d=s.block3d,
+                         k_scale=k_scale, v_scale=v_scale)
+        li.li_quantize_pages(ctx, kc, vc, torch.arange(s.n_pages, dtype=torch.int32, device=dev))
+        kcur_dev, vcur_dev = kc[cur_pages].contiguous(), vc[cur_pages].contiguous()
+        cur_idx32 = torch.tensor(cur_pages, dtype=torch.int32, device=dev)
+        del kc, vc
+        args.no_extras = True
+    else:
+        ctx = li.Context(q, kc, vc, fi, prob.frame_off, s.n_cur_frames, s.block, grid=s.grid, block3d=s.block3d)
     buf = li.Buffers(ctx, prob.kmax, want_scores=False, want_lse=True)
     o_host = torch.empty(buf.o.shape, dtype=buf.o.dtype).pin_memory()
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)   # > 126 MB L2
@@ -237,7 +252,11 @@ def run_cuda(args):
     def e2e_step():
         q.copy_(q_host, non_blocking=True)
         fi.copy_(fi_host, non_blocking=True)
-        if contiguous_cur:
+        if fp8:
+            kcur_dev.copy_(kcur_host, non_blocking=True)
+            vcur_dev.copy_(vcur_host, non_blocking=True)
+            li.li_quantize_pages(ctx, kcur_dev, vcur_dev, cur_idx32, stream)
+        elif contiguous_cur:
             kc[cur_pages[0]:cur_pages[-1] + 1].copy_(kcur_host, non_blocking=True)
             vc[cur_pages[0]:cur_pages[-1] + 1].copy_(vcur_host, non_blocking=True)
         else:
@@ -252,7 +271,7 @@ def run_cuda(args):
     # computed and read back group by group on three streams, so that host->device copies, kernels and the
     # device->host copy of O overlap inside ONE step.  Same work, same bytes, same C-ABI calls (on head slices).
     # Needs B == 1 (a head slice of O is then contiguous); otherwise the plain sequence above is used.
-    G = args.e2e_groups if (prob.B == 1 and args.e2e_groups > 1 and s.H % args.e2e_groups == 0) else 1
+    G = args.e2e_groups if (prob.B == 1 and args.e2e_groups > 1 and s.H % args.e2e_groups == 0 and not fp8) else 1
     if G > 1:
         Hg = s.H // G
         hs = [slice(g * Hg, (g + 1) * Hg) for g in range(G)]
@@ -460,24 +479,28 @@ def run_cuda(args):
         value = job_throughput(flops, args.steps, world, total_ms)
         e2e_val = job_throughput(flops, args.steps, world, e2e_ms)
         attn_tflops = flops / (float(att_ms.mean()) * 1e-3) / 1e12
-        sel_bytes = sum((prob.Lq + prob.L_hist(b)) * s.d * 2 * s.H for b in range(prob.B))
+        # FP8 pages: the tensor roofline is the fp8 one = the measured bf16 peak x the guide's nominal ratio (2x); the
+        # select kernels read Q in bf16 and the historical K in one byte per element
+        tpeak = pk["bf16_tflops"] * (2.0 if fp8 else 1.0)
+        sel_bytes = sum((2 * prob.Lq + (1 if fp8 else 2) * prob.L_hist(b)) * s.d * s.H for b in range(prob.B))
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
             "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "bf16", "data": "synthetic",
+            "dtype": "fp8-e4m3 (K/V pages, Q rows and probabilities; fp32 accumulation)" if fp8 else "bf16", "data": "synthetic",
             "config": {"workload": s.name, "B": prob.B, "H": s.H, "d": s.d, "Lq": prob.Lq, "frame_tokens": s.frame_tokens,
-                       "block": s.block, "block3d": s.block3d, "grid": s.grid, "Lk": [prob.L_hist(b) + prob.Lq for b in range(prob.B)],
+                       "block": s.block, "block3d": s.block3d, "grid": s.grid, "kv": args.kv, "Lk": [prob.L_hist(b) + prob.Lq for b in range(prob.B)],
                        "top_k": [int(x) for x in prob.top_k], "M": [prob.M(b) for b in range(prob.B)],
                        "l2": "flushed between timed steps (256 MiB write)", "multi_gpu": "replicas only (no collective)"},
             "effective_flops_per_step": int(flops),
             "select_ms": float(sel_ms.mean()), "attn_ms": float(att_ms.mean()), "attn_ms_min": float(att_ms.min()),
             "select_overhead_frac_of_attn": float(sel_ms.mean() / att_ms.mean()),
             "select_gbs": sel_bytes / (float(sel_ms.mean()) * 1e-3) / 1e9,
-            "frac_of_peak_burst": attn_tflops / pk["bf16_tflops"], "frac_of_peak_sustained": attn_tflops / pk["bf16_tflops_sustained"],
-            "roofline": {"bound": "tensor", "achieved": attn_tflops, "peak": pk["bf16_tflops"], "unit": "TFLOP/s",
-                         "frac": attn_tflops / pk["bf16_tflops"], "traffic": ncu_traffic(s.name)[0],
-                         "traffic_source": ncu_traffic(s.name)[1],
-                         "kernel": "li_sparse_attn_kernel", "peak_source": pk["source"] + " burst bf16"},
+            "frac_of_peak_burst": attn_tflops / tpeak, "frac_of_peak_sustained": attn_tflops / (pk["bf16_tflops_sustained"] * (2.0 if fp8 else 1.0)),
+            "roofline": {"bound": "tensor", "achieved": attn_tflops, "peak": tpeak, "unit": "TFLOP/s",
+                         "frac": attn_tflops / tpeak, "traffic": None if fp8 else ncu_traffic(s.name)[0],
+                         "traffic_source": None if fp8 else ncu_traffic(s.name)[1],
+                         "kernel": "li_sparse_attn_fp8_kernel" if fp8 else "li_sparse_attn_kernel",
+                         "peak_source": pk["source"] + (" burst bf16 x 2 (nominal fp8 : bf16 ratio)" if fp8 else " burst bf16")},
             "roofline_select": {"bound": "hbm", "achieved": sel_bytes / (float(sel_ms.mean()) * 1e-3) / 1e9, "peak": pk["hbm_gbs"],
                                 "unit": "GB/s", "frac": sel_bytes / (float(sel_ms.mean()) * 1e-3) / 1e9 / pk["hbm_gbs"],
                                 "kernel": "li_pool_kernel + li_score_topk_kernel"},
@@ -490,7 +513,7 @@ def run_cuda(args):
             "gpu_launches": int(launches), "clocks": clk.summary(),
         }
         line.update(extras)
-        if not args.no_cpu and world == 1:
+        if not args.no_cpu and world == 1 and not fp8:
             dt, fl, desc = oracle_sample(prob, args.ref_heads, args.ref_tiles)
             line["cpu_baseline"] = {"value": fl / dt / 1e12, "unit": UNIT, "cores": cpu_threads(), "kind": "oracle",
                                     "sample": desc, "seconds": dt}
@@ -508,6 +531,7 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--e2e-groups", type=int, default=4, help="head groups the end-to-end leg is pipelined over (1 = plain sequence)")
     ap.add_argument("--config", default="mid", choices=["tiny", "mid", "long", "adaptive", "dense-equivalence", "mid3d", "long3d", "mid3d448"])
+    ap.add_argument("--kv", default="bf16", choices=["bf16", "fp8"], help="precision of the K/V pages (fp8: E4M3 codes + per-head scales)")
     ap.add_argument("--ref-heads", type=int, default=24, help="heads in the oracle's bounded sample")
     ap.add_argument("--ref-tiles", type=int, default=None, help="query blocks per head in the oracle's sample (default all)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")

@@ -52,6 +52,7 @@ enum {
 
 /* li_problem.flags */
 #define LI_FLAG_NO_SPLIT 1u     /* li_sparse_attn: never split the query blocks of the last wave */
+#define LI_FLAG_KV_FP8   2u     /* k_cache / v_cache hold FP8 E4M3 codes, see k_scale / v_scale below */
 
 typedef struct li_problem {
   int32_t B, H, Lq, d;          /* B independent calls; Lq = n_cur_frames * frame_tokens when n_cur_frames > 0 */
@@ -85,6 +86,15 @@ typedef struct li_problem {
   const void *text_v;           /* bf16, same shape and strides */
   int64_t t_sb, t_sh, t_st;     /* batch / head / token strides of both */
   uint32_t flags;               /* LI_FLAG_* bits, 0 = defaults */
+  /* FP8 K/V pages (LI_FLAG_KV_FP8; the paper states no cache precision): k_cache and
+   * v_cache are uint8 [n_pages,H,T_f,d] of OCP FP8 E4M3 codes (1-4-3, bias 7, no infinities, max 448), strides in
+   * elements (= bytes, multiples of 16), value = decode(code) * scale[h] with one fp32 scale per head.  Pages are written
+   * by li_quantize_pages.  li_block_select pools the dequantised K; li_sparse_attn replaces every query row by its own
+   * e4m3 image (scale max|q_u| / 448, fp32) and runs both contractions on the FP8 tensor-core path, the probabilities
+   * rounded to e4m3.  Supported: d == 128, block 128, no text prefix, 1-D or 3-D blocks; li_pool_pages /
+   * li_block_select_cached are bf16-only. */
+  const float *k_scale;         /* DEVICE fp32 [H] */
+  const float *v_scale;         /* DEVICE fp32 [H] */
 } li_problem;
 
 /* Eq. 9-10.  For every call b, head h and query block i: pooled means (true cardinality
@@ -140,6 +150,13 @@ int li_block_select_cached(const li_problem *p, const int32_t *top_k_host, int32
  *               (results equal up to fp32 rounding of the merge).  NULL or a smaller buffer: never split. */
 int li_sparse_attn(const li_problem *p, const int32_t *sel_idx, const int32_t *sel_cnt, int32_t kmax,
                    void *o, float *lse_opt, void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* Quantise-on-write for FP8 pages (LI_FLAG_KV_FP8 must be set in p): for t in [0, n_list) page pages_dev[t] of
+ * p->k_cache / p->v_cache receives encode(src[t] / scale[h]) -- division in fp32, round to nearest even, saturating at
+ * +-448 (PTX cvt.rn.satfinite.e4m3x2.f32) -- of the bf16 rows k_src / v_src [n_list,H,T_f,d] (contiguous, 16-byte
+ * aligned).  HBM-bound: reads 4 and writes 2 bytes per element pair.  Page ids outside [0, n_pages) are skipped. */
+int li_quantize_pages(const li_problem *p, const void *k_src, const void *v_src, const int32_t *pages_dev, int32_t n_list,
+                      void *cuda_stream);
 
 /* Debug validation of DEVICE-side inputs that the calls above trust (one small launch, asynchronous, no host
  * synchronisation; meant for debug builds of the caller, not for the hot loop):

@@ -19,10 +19,11 @@ LIB_PATH = os.path.join(_HERE, "libli.so")
 LI_OK, LI_ERR_INVALID_ARG, LI_ERR_UNSUPPORTED, LI_ERR_WORKSPACE, LI_ERR_CUDA = 0, -1, -2, -3, -4
 LI_MAX_CALLS = 64
 LI_FLAG_NO_SPLIT = 1
+LI_FLAG_KV_FP8 = 2
 LI_BAD_PAGE_ID, LI_BAD_SEL_CNT, LI_BAD_SEL_RANGE, LI_BAD_SEL_DUPLICATE = 1, 2, 4, 8
 
 EXPORTS = ("li_block_select", "li_block_select_reuse_kbar", "li_block_select_cached", "li_pool_pages", "li_slice_cache_bytes",
-           "li_sparse_attn", "li_validate", "li_workspace_bytes", "li_context_policy",
+           "li_sparse_attn", "li_validate", "li_quantize_pages", "li_workspace_bytes", "li_context_policy",
            "li_policy_workspace_bytes", "li_launch_count", "li_reset_launch_count", "li_strerror", "li_version",
            "li_last_cuda_error")
 
@@ -50,6 +51,7 @@ class li_problem(ctypes.Structure):
         ("Lt", ctypes.c_int32), ("text_k", ctypes.c_void_p), ("text_v", ctypes.c_void_p),
         ("t_sb", ctypes.c_int64), ("t_sh", ctypes.c_int64), ("t_st", ctypes.c_int64),
         ("flags", ctypes.c_uint32),
+        ("k_scale", ctypes.c_void_p), ("v_scale", ctypes.c_void_p),
     ]
 
 
@@ -108,6 +110,8 @@ def lib() -> ctypes.CDLL:
         L.li_context_policy.restype = ctypes.c_int
         L.li_context_policy.argtypes = [ctypes.POINTER(li_policy), ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p,
                                         ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p]
+        L.li_quantize_pages.restype = ctypes.c_int
+        L.li_quantize_pages.argtypes = [P, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p]
         L.li_validate.restype = ctypes.c_int
         L.li_validate.argtypes = [P, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p, ctypes.c_void_p]
         L.li_last_cuda_error.restype = ctypes.c_int
@@ -143,10 +147,20 @@ class Context:
     def __init__(self, q: torch.Tensor, k_cache: torch.Tensor, v_cache: torch.Tensor, frame_idx: torch.Tensor,
                  frame_off: Sequence[int], n_cur_frames: int, block: int, softmax_scale: float = 0.0,
                  grid: Optional[Tuple[int, int]] = None, block3d: Optional[Tuple[int, int, int]] = None,
-                 text_k: Optional[torch.Tensor] = None, text_v: Optional[torch.Tensor] = None, flags: int = 0):
-        for t, name in ((q, "q"), (k_cache, "k_cache"), (v_cache, "v_cache")):
-            if t.dtype != torch.bfloat16 or not t.is_cuda or t.dim() != 4 or t.stride(-1) != 1:
-                raise ValueError(f"{name} must be a 4-D CUDA bf16 tensor with unit innermost stride")
+                 text_k: Optional[torch.Tensor] = None, text_v: Optional[torch.Tensor] = None, flags: int = 0,
+                 k_scale: Optional[torch.Tensor] = None, v_scale: Optional[torch.Tensor] = None):
+        """k_cache / v_cache: bf16, or uint8 FP8-E4M3 codes together with k_scale / v_scale (fp32 CUDA tensors [H])."""
+        fp8 = k_cache.dtype == torch.uint8
+        for t, name, dt in ((q, "q", torch.bfloat16), (k_cache, "k_cache", torch.uint8 if fp8 else torch.bfloat16),
+                            (v_cache, "v_cache", torch.uint8 if fp8 else torch.bfloat16)):
+            if t.dtype != dt or not t.is_cuda or t.dim() != 4 or t.stride(-1) != 1:
+                raise ValueError(f"{name} must be a 4-D CUDA {dt} tensor with unit innermost stride")
+        if fp8:
+            for t, name in ((k_scale, "k_scale"), (v_scale, "v_scale")):
+                if t is None or t.dtype != torch.float32 or not t.is_cuda or not t.is_contiguous() or t.numel() != q.shape[1]:
+                    raise ValueError(f"{name} must be a contiguous fp32 CUDA tensor of H entries")
+            flags |= LI_FLAG_KV_FP8
+        self.k_scale, self.v_scale = k_scale, v_scale
         if k_cache.shape != v_cache.shape or k_cache.stride() != v_cache.stride():
             raise ValueError("k_cache and v_cache must have the same shape and strides")
         if frame_idx.dtype != torch.int32 or not frame_idx.is_cuda or not frame_idx.is_contiguous():
@@ -170,6 +184,8 @@ class Context:
         p.n_cur_frames = n_cur_frames
         p.softmax_scale = softmax_scale
         p.flags = int(flags)
+        if fp8:
+            p.k_scale, p.v_scale = k_scale.data_ptr(), v_scale.data_ptr()
         self.text_k, self.text_v = text_k, text_v
         if text_k is not None:
             for t, name in ((text_k, "text_k"), (text_v, "text_v")):
@@ -271,6 +287,21 @@ def li_sparse_attn(ctx: Context, sel_idx: torch.Tensor, sel_cnt: torch.Tensor, k
                               _stream_ptr(stream))
     if rc != LI_OK:
         raise LiError(rc, "li_sparse_attn")
+
+
+def li_quantize_pages(ctx: Context, k_src: torch.Tensor, v_src: torch.Tensor, pages: torch.Tensor,
+                      stream: Optional[torch.cuda.Stream] = None) -> None:
+    """li_quantize_pages (include/li.h): bf16 rows [n_list,H,T_f,d] -> the FP8 pages `pages` (int32 CUDA) of ctx's caches."""
+    for t in (k_src, v_src):
+        if t.dtype != torch.bfloat16 or not t.is_cuda or not t.is_contiguous() or t.shape[1:] != ctx.k_cache.shape[1:] or \
+                t.shape[0] != pages.numel():
+            raise ValueError("k_src / v_src must be contiguous bf16 CUDA tensors [n_list,H,T_f,d]")
+    if pages.dtype != torch.int32 or not pages.is_cuda or not pages.is_contiguous():
+        raise ValueError("pages must be a contiguous int32 CUDA tensor")
+    rc = lib().li_quantize_pages(ctypes.byref(ctx.p), k_src.data_ptr(), v_src.data_ptr(), pages.data_ptr(), pages.numel(),
+                                 _stream_ptr(stream))
+    if rc != LI_OK:
+        raise LiError(rc, "li_quantize_pages")
 
 
 def li_validate(ctx: Context, error: torch.Tensor, sel_idx: Optional[torch.Tensor] = None,

@@ -9,7 +9,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libli.so")
-SOURCES = ["li_api.cu", "li_select.cu", "li_attn.cu", "li_policy.cu"]
+SOURCES = ["li_api.cu", "li_select.cu", "li_attn.cu", "li_policy.cu", "li_fp8.cu"]
 HEADERS = ["li_internal.h", "li_ptx.cuh", os.path.join("..", "..", "include", "li.h")]
 
 

@@ -40,7 +40,7 @@ EncodeFn get_encode() {
 // same tensors as an earlier one (the steady state of an AR loop) does no driver work.
 struct MapKey {
   const void *base;
-  int32_t rank, d, box[4];
+  int32_t rank, d, box[4], elem_bytes;   // elem_bytes: 2 = bf16 (inner box 64 elements), 1 = FP8 codes (inner box 128)
   int64_t dims[4], strides[4];
   bool operator==(const MapKey &o) const { return std::memcmp(this, &o, sizeof(MapKey)) == 0; }
 };
@@ -63,13 +63,14 @@ bool encode_cached(CUtensorMap *tm, const MapKey &key) {
   if (enc == nullptr) return false;
   cuuint64_t dims[5] = {(cuuint64_t)key.d};
   cuuint64_t strides[4];
-  cuuint32_t box[5] = {64}, estr[5] = {1, 1, 1, 1, 1};
+  cuuint32_t box[5] = {(cuuint32_t)(128 / key.elem_bytes)}, estr[5] = {1, 1, 1, 1, 1};   // 128 bytes = the swizzle span
   for (int k = 0; k + 1 < key.rank; ++k) {
     dims[k + 1] = (cuuint64_t)key.dims[k];
-    strides[k] = (cuuint64_t)key.strides[k] * 2;
+    strides[k] = (cuuint64_t)key.strides[k] * key.elem_bytes;
     box[k + 1] = (cuuint32_t)key.box[k];
   }
-  CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, (cuuint32_t)key.rank, const_cast<void *>(key.base), dims, strides, box,
+  CUresult r = enc(tm, key.elem_bytes == 1 ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16,
+                   (cuuint32_t)key.rank, const_cast<void *>(key.base), dims, strides, box,
                    estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return false;
@@ -83,10 +84,10 @@ bool encode_cached(CUtensorMap *tm, const MapKey &key) {
 // bf16 tensor [n3, n2, n1, d] (innermost first: d, n1, n2, n3), strides in elements, box = 64 x rows x 1 x 1,
 // SWIZZLE_128B, out-of-bounds elements read as zero.
 bool encode_map(CUtensorMap *tm, const void *base, int d, int64_t n1, int64_t n2, int64_t n3, int64_t s1, int64_t s2,
-                int64_t s3, int box_rows) {
+                int64_t s3, int box_rows, int elem_bytes = 2) {
   MapKey k;
   std::memset(&k, 0, sizeof(k));
-  k.base = base; k.rank = 4; k.d = d;
+  k.base = base; k.rank = 4; k.d = d; k.elem_bytes = elem_bytes;
   k.dims[0] = n1; k.dims[1] = n2; k.dims[2] = n3;
   k.strides[0] = s1; k.strides[1] = s2; k.strides[2] = s3;
   k.box[0] = box_rows; k.box[1] = 1; k.box[2] = 1;
@@ -96,10 +97,10 @@ bool encode_map(CUtensorMap *tm, const void *base, int d, int64_t n1, int64_t n2
 // bf16 tensor viewed as 5-D [n4, n3, gh, gw, d] (innermost first: d, gw, gh, n3, n4), box = 64 x bw x bh x 1 x 1:
 // one frame's bh x bw patch of a 3-D block = 32 rows of 128 bytes, SWIZZLE_128B, zero fill outside.
 bool encode_map5(CUtensorMap *tm, const void *base, int d, int gw, int gh, int64_t n3, int64_t n4, int64_t s_w,
-                 int64_t s_h, int64_t s3, int64_t s4, int bw, int bh) {
+                 int64_t s_h, int64_t s3, int64_t s4, int bw, int bh, int elem_bytes = 2) {
   MapKey k;
   std::memset(&k, 0, sizeof(k));
-  k.base = base; k.rank = 5; k.d = d;
+  k.base = base; k.rank = 5; k.d = d; k.elem_bytes = elem_bytes;
   k.dims[0] = gw; k.dims[1] = gh; k.dims[2] = n3; k.dims[3] = n4;
   k.strides[0] = s_w; k.strides[1] = s_h; k.strides[2] = s3; k.strides[3] = s4;
   k.box[0] = bw; k.box[1] = bh; k.box[2] = 1; k.box[3] = 1;
@@ -155,6 +156,11 @@ int check_problem(const li_problem *p, Derived *dv, bool pages_only = false) {
     if (s <= 0 || s % 8 != 0) return LI_ERR_INVALID_ARG;
   if (p->q_st < p->d || p->kv_st < p->d) return LI_ERR_INVALID_ARG;
   if (((uintptr_t)p->q | (uintptr_t)p->k_cache | (uintptr_t)p->v_cache) & 15u) return LI_ERR_INVALID_ARG;
+  if (p->flags & LI_FLAG_KV_FP8) {
+    if (p->d != 128 || p->block_k != 128 || p->Lt != 0) return LI_ERR_UNSUPPORTED;
+    if (p->k_scale == nullptr || p->v_scale == nullptr) return LI_ERR_INVALID_ARG;
+    if (p->kv_sp % 16 != 0 || p->kv_sh % 16 != 0 || p->kv_st % 16 != 0) return LI_ERR_INVALID_ARG;   // byte strides (TMA: 16)
+  }
   if (p->Lt < 0) return LI_ERR_INVALID_ARG;
   if (p->Lt > 0) {
     if (p->text_k == nullptr || p->text_v == nullptr) return LI_ERR_INVALID_ARG;
@@ -224,6 +230,7 @@ static int block_select_impl(const li_problem *p, const int32_t *top_k_host, int
   int rc = check_problem(p, &dv);
   if (rc != LI_OK) return rc;
   if (slice_cache != nullptr && dv.tl.bt == 0) return LI_ERR_UNSUPPORTED;   // patch sums exist for 3-D blocks only
+  if (slice_cache != nullptr && (p->flags & LI_FLAG_KV_FP8)) return LI_ERR_UNSUPPORTED;   // ... and for bf16 pages only
   if (top_k_host == nullptr || sel_idx == nullptr || sel_cnt == nullptr || kmax < 1) return LI_ERR_INVALID_ARG;
   if (scores_opt != nullptr && score_pitch < dv.Mmax) return LI_ERR_INVALID_ARG;
   if (workspace == nullptr || workspace_bytes < ws_bytes(p, dv) + ws_split_bytes(p) || ((uintptr_t)workspace & 255u))
@@ -256,6 +263,7 @@ static int block_select_impl(const li_problem *p, const int32_t *top_k_host, int
   int64_t n = 0;
   int e = 0;
   sp.slice_cache = slice_cache;             // non-null: the pool kernel forms kbar from the cached patch sums
+  sp.k_scale = (p->flags & LI_FLAG_KV_FP8) ? p->k_scale : nullptr;
   e = li::launch_select(sp, dv.meta, (cudaStream_t)cuda_stream, &n);
   g_launches += n;
   return e == 0 ? LI_OK : cuda_failed(e);
@@ -271,6 +279,7 @@ int li_pool_pages(const li_problem *p, const int32_t *pages_dev, int32_t n_list,
   Derived dv;
   int rc = check_problem(p, &dv, true);
   if (rc != LI_OK) return rc;
+  if (p->flags & LI_FLAG_KV_FP8) return LI_ERR_UNSUPPORTED;
   if (n_list < 0 || slice_cache == nullptr || (n_list > 0 && pages_dev == nullptr) || ((uintptr_t)slice_cache & 15u))
     return LI_ERR_INVALID_ARG;
   li::SelectParams sp;
@@ -323,25 +332,26 @@ int li_sparse_attn(const li_problem *p, const int32_t *sel_idx, const int32_t *s
   const int has_full = p->frame_tokens >= half ? 1 : 0;
   CUtensorMap tm_q, tm_kf, tm_k8, tm_vf, tm_v8;
   bool ok;
+  const int eb = (p->flags & LI_FLAG_KV_FP8) ? 1 : 2;      // bytes per K/V element
   if (dv.tl.bt > 0) {
     // 3-D blocks: 5-D maps (d, grid column, grid row, head | frame, page | batch*head)
     const int gw = p->grid_w, gh = p->grid_h;
     ok = encode_map5(&tm_q, p->q, p->d, gw, gh, p->Lq / p->frame_tokens, (int64_t)p->B * p->H, p->q_st, gw * p->q_st,
                      (int64_t)p->frame_tokens * p->q_st, p->q_sh, p->bw, p->bh);
     ok = ok && encode_map5(&tm_kf, p->k_cache, p->d, gw, gh, p->H, p->n_pages, p->kv_st, gw * p->kv_st, p->kv_sh,
-                           p->kv_sp, p->bw, p->bh);
+                           p->kv_sp, p->bw, p->bh, eb);
     ok = ok && encode_map5(&tm_vf, p->v_cache, p->d, gw, gh, p->H, p->n_pages, p->kv_st, gw * p->kv_st, p->kv_sh,
-                           p->kv_sp, p->bw, p->bh);
+                           p->kv_sp, p->bw, p->bh, eb);
     tm_k8 = tm_kf;
     tm_v8 = tm_vf;
   } else {
     ok = encode_map(&tm_q, p->q, p->d, p->Lq, p->H, p->B, p->q_st, p->q_sh, p->q_sb, blk);
-    ok = ok && encode_map(&tm_k8, p->k_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp, 8);
-    ok = ok && encode_map(&tm_v8, p->v_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp, 8);
+    ok = ok && encode_map(&tm_k8, p->k_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp, 8, eb);
+    ok = ok && encode_map(&tm_v8, p->v_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp, 8, eb);
     ok = ok && encode_map(&tm_kf, p->k_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp,
-                          has_full ? half : 8);
+                          has_full ? half : 8, eb);
     ok = ok && encode_map(&tm_vf, p->v_cache, p->d, p->frame_tokens, p->H, p->n_pages, p->kv_st, p->kv_sh, p->kv_sp,
-                          has_full ? half : 8);
+                          has_full ? half : 8, eb);
   }
   CUtensorMap tm_tk = tm_q, tm_tv = tm_q;      // placeholders when there is no text
   if (p->Lt > 0) {
@@ -356,6 +366,7 @@ int li_sparse_attn(const li_problem *p, const int32_t *sel_idx, const int32_t *s
   ap.B = p->B; ap.H = p->H; ap.Lq = p->Lq; ap.T_f = p->frame_tokens; ap.n_cur = p->n_cur_frames;
   ap.Nqb = dv.Nqb; ap.Nc = dv.Nc; ap.kmax = kmax; ap.has_box_full = has_full; ap.Lt = p->Lt;
   ap.no_split = (p->flags & LI_FLAG_NO_SPLIT) ? 1 : 0;
+  if (p->flags & LI_FLAG_KV_FP8) { ap.k_scale = p->k_scale; ap.v_scale = p->v_scale; }
   const float scale = p->softmax_scale != 0.f ? p->softmax_scale : 1.0f / std::sqrt((float)p->d);
   ap.scale_log2 = scale * 1.4426950408889634f;
   ap.frame_idx = p->frame_idx; ap.sel_idx = sel_idx; ap.sel_cnt = sel_cnt;
@@ -366,6 +377,29 @@ int li_sparse_attn(const li_problem *p, const int32_t *sel_idx, const int32_t *s
   }
   int64_t n = 0;
   const int e = li::launch_attn(ap, dv.meta, p->d, blk, tm_q, tm_tk, tm_tv, tm_kf, tm_k8, tm_vf, tm_v8, (cudaStream_t)cuda_stream, &n);
+  g_launches += n;
+  return e == 0 ? LI_OK : cuda_failed(e);
+}
+
+int li_quantize_pages(const li_problem *p, const void *k_src, const void *v_src, const int32_t *pages_dev, int32_t n_list,
+                      void *cuda_stream) {
+  if (p == nullptr || !(p->flags & LI_FLAG_KV_FP8)) return LI_ERR_INVALID_ARG;
+  if (p->H <= 0 || p->frame_tokens <= 0 || p->n_pages <= 0 || p->k_cache == nullptr || p->v_cache == nullptr ||
+      p->k_scale == nullptr || p->v_scale == nullptr)
+    return LI_ERR_INVALID_ARG;
+  if (p->d != 128) return LI_ERR_UNSUPPORTED;
+  if (n_list < 0 || (n_list > 0 && (k_src == nullptr || v_src == nullptr || pages_dev == nullptr))) return LI_ERR_INVALID_ARG;
+  if ((((uintptr_t)k_src | (uintptr_t)v_src | (uintptr_t)p->k_cache | (uintptr_t)p->v_cache) & 15u) != 0) return LI_ERR_INVALID_ARG;
+  if (p->kv_sp % 16 != 0 || p->kv_sh % 16 != 0 || p->kv_st % 16 != 0 || p->kv_st < p->d) return LI_ERR_INVALID_ARG;
+  li::QuantParams qp;
+  std::memset(&qp, 0, sizeof(qp));
+  qp.H = p->H; qp.T_f = p->frame_tokens; qp.d = p->d; qp.n_pages = p->n_pages;
+  qp.k_src = (const uint16_t *)k_src; qp.v_src = (const uint16_t *)v_src;
+  qp.k_cache = (uint8_t *)const_cast<void *>(p->k_cache); qp.v_cache = (uint8_t *)const_cast<void *>(p->v_cache);
+  qp.kv_sp = p->kv_sp; qp.kv_sh = p->kv_sh; qp.kv_st = p->kv_st;
+  qp.k_scale = p->k_scale; qp.v_scale = p->v_scale; qp.pages = pages_dev;
+  int64_t n = 0;
+  const int e = li::launch_quantize_pages(qp, n_list, (cudaStream_t)cuda_stream, &n);
   g_launches += n;
   return e == 0 ? LI_OK : cuda_failed(e);
 }

@@ -37,16 +37,19 @@ constexpr float kRescaleThreshold = 8.0f;   // log2 units: P stays <= 2^8 betwee
 #endif
 constexpr int kEmuOf4 = LI_EMU_OF_4;        // of every 4 column pairs, how many use the FMA-pipe exp2
 
-template <int D, int BLK>
+template <int D, int BLK, bool KV8 = false>
 struct AttnSmem {
   static constexpr int HALF = BLK / 2;
-  static constexpr int kQChunk = 128 * 128;            // bytes of one 64-column chunk of the 128-row Q tile
-  static constexpr int kKVChunk = HALF * 128;          // bytes of one 64-column chunk of a K or V half-tile
+  static constexpr int kQChunk = 128 * 128;            // bytes of one 64-column chunk of the 128-row (bf16) Q tile
+  static constexpr int kKVChunk = HALF * 128;          // bytes of one 128-byte-wide chunk of a K or V half-tile
+  static constexpr int kKVChunks = KV8 ? D / 128 : D / 64;   // 128 bytes = 64 bf16 channels or 128 e4m3 channels
   static constexpr int kQ = (D / 64) * kQChunk;
-  static constexpr int kStage = (D / 64) * kKVChunk;
+  static constexpr int kQ8 = KV8 ? 128 * 128 : 0;      // FP8 pages: the e4m3 image of the Q tile (128 rows x 128 bytes)
+  static constexpr int kStage = kKVChunks * kKVChunk;
   static constexpr int kOffQ = 0;
-  static constexpr int kOffRing = kQ;
-  static constexpr int kOffSel = kQ + kStages * kStage;
+  static constexpr int kOffQ8 = kQ;
+  static constexpr int kOffRing = kQ + kQ8;
+  static constexpr int kOffSel = kOffRing + kStages * kStage;
   static constexpr int kOffPages = kOffSel + kSelCap * 4;   // this call's frame list, staged once
   static constexpr int kOffInfo = kOffPages + kPageCap * 4;  // 3-D: per attended tile (frames present) | (valid rows per slice) << 8
   static constexpr int kOffBar = kOffInfo + kInfoCap * 2;
@@ -61,6 +64,7 @@ enum {
   BAR_P_FULL = BAR_S_FULL + 2,       // +buffer
   BAR_PV_DONE = BAR_P_FULL + 2,
   BAR_O_FULL,
+  BAR_Q8,                            // FP8 pages: the softmax warps have written the e4m3 image of Q
   BAR_COUNT
 };
 
@@ -89,13 +93,16 @@ __device__ __forceinline__ int64_t row_token(const AttnParams &p, int i, int row
   return row < min(BLK, p.Lq - i * BLK) ? (int64_t)i * BLK + row : -1;
 }
 
-template <int D, int BLK, bool K3D, bool TEXT, bool SPLIT>
+template <int D, int BLK, bool K3D, bool TEXT, bool SPLIT, bool KV8>
 __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &meta, const CUtensorMap &tm_q,
                                           const CUtensorMap &tm_k_full, const CUtensorMap &tm_k_8,
                                           const CUtensorMap &tm_v_full, const CUtensorMap &tm_v_8,
                                           const CUtensorMap &tm_tk, const CUtensorMap &tm_tv) {
-  using L = AttnSmem<D, BLK>;
+  using L = AttnSmem<D, BLK, KV8>;
   constexpr int HALF = L::HALF;
+  constexpr int KCH = L::kKVChunks, CW = KV8 ? 128 : 64;   // K/V chunks per half-tile, channels per chunk
+  constexpr int EB = KV8 ? 1 : 2;                          // bytes per K/V element
+  static_assert(!KV8 || (D == 128 && !TEXT), "FP8 pages: d = 128, no text prefix");
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   uint8_t *smem = smem_raw + (smem_base - smem_u32(smem_raw));
@@ -158,7 +165,7 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
       tma_prefetch_desc(&tm_tk);
       tma_prefetch_desc(&tm_tv);
     }
-    for (int k = 0; k < BAR_COUNT; ++k) mbar_init(bar(k), (k == BAR_P_FULL || k == BAR_P_FULL + 1) ? 4 : 1);
+    for (int k = 0; k < BAR_COUNT; ++k) mbar_init(bar(k), (k == BAR_P_FULL || k == BAR_P_FULL + 1 || k == BAR_Q8) ? 4 : 1);
     *sT = 0;
     *sTailPos = -1;
     mbar_fence_init();
@@ -279,7 +286,7 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
           if (elect_one()) {
             mbar_arrive_expect_tx(mb, HALF * D * 2);
 #pragma unroll
-            for (int c = 0; c < D / 64; ++c) tma_load_4d(dst + c * L::kKVChunk, tm_text, mb, c * 64, j * BLK + hh * HALF, h, b);
+            for (int c = 0; c < D / 64; ++c) tma_load_4d(dst + c * L::kKVChunk, tm_text, mb, c * 64, j * BLK + hh * HALF, h, b);   // text: bf16 only
           }
           __syncwarp();
           ++n;
@@ -301,12 +308,12 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
           }
           mbar_wait(bar(BAR_EMPTY + slot), ((n >> 2) & 1) ^ 1);
           if (elect_one()) {
-            mbar_arrive_expect_tx(mb, HALF * D * 2);
+            mbar_arrive_expect_tx(mb, HALF * D * EB);
 #pragma unroll
             for (int s = 0; s < SPH; ++s)
 #pragma unroll
-              for (int c = 0; c < D / 64; ++c)
-                tma_load_5d(dst + c * L::kKVChunk + s * 4096, tm_full, mb, c * 64, wb * tl.bw, y0[s], h, pg[s]);
+              for (int c = 0; c < KCH; ++c)
+                tma_load_5d(dst + c * L::kKVChunk + s * 4096, tm_full, mb, c * CW, wb * tl.bw, y0[s], h, pg[s]);
           }
           __syncwarp();
           ++n;
@@ -320,13 +327,13 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
         const int page0 = page_at(f0 + pg0);
         mbar_wait(bar(BAR_EMPTY + slot), ((n >> 2) & 1) ^ 1);
         if (elect_one()) {
-          mbar_arrive_expect_tx(mb, HALF * D * 2);
+          mbar_arrive_expect_tx(mb, HALF * D * EB);
           if (one_page) {
-            // inside one page: one box per 64-column chunk; rows past the page end are zero-filled by the
+            // inside one page: one box per 128-byte chunk; rows past the page end are zero-filled by the
             // hardware (a region always ends on a page boundary)
             const int row = t0 - pg0 * p.T_f;
 #pragma unroll
-            for (int c = 0; c < D / 64; ++c) tma_load_4d(dst + c * L::kKVChunk, tm_full, mb, c * 64, row, h, page0);
+            for (int c = 0; c < KCH; ++c) tma_load_4d(dst + c * L::kKVChunk, tm_full, mb, c * CW, row, h, page0);
           } else {
             // straddles frames: 8-row pieces (one SWIZZLE_128B atom each, destinations stay 1024-B aligned)
             int cur_pg = pg0, page = page0;
@@ -339,8 +346,8 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
                 row = tt - pg * p.T_f;
               }
 #pragma unroll
-              for (int c = 0; c < D / 64; ++c)
-                tma_load_4d(dst + c * L::kKVChunk + g * 1024, tm_8, mb, c * 64, row, h, page);
+              for (int c = 0; c < KCH; ++c)
+                tma_load_4d(dst + c * L::kKVChunk + g * 1024, tm_8, mb, c * CW, row, h, page);
             }
           }
         }
@@ -368,8 +375,9 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
       // =============================== MMA issuer ===============================
       // The whole warp walks the loop converged (barrier waits, descriptor arithmetic on warp-uniform values);
       // one elected lane issues the tcgen05 instructions.
-      constexpr uint32_t idesc_qk = idesc_bf16(128, HALF, 0);
-      constexpr uint32_t idesc_pv = idesc_bf16(128, D, 1);
+      constexpr uint32_t idesc_qk = KV8 ? idesc_e4m3(128, HALF, 0) : idesc_bf16(128, HALF, 0);
+      constexpr uint32_t idesc_pv = KV8 ? idesc_e4m3(128, D, 1) : idesc_bf16(128, D, 1);
+      const uint32_t sQ8 = smem_base + L::kOffQ8;
       int c = 0;                                     // running consume index: slot = c % 4
       auto issue_qk = [&](int t) {
         const int slot = c & (kStages - 1);
@@ -379,18 +387,25 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
         if (elect_one()) {
           // descriptors of the kk-th 16-channel slice: the start address (16-byte units, cannot carry out of its
           // field) advances by 32 B inside the 128-B row and by one 64-channel chunk every 4 slices
-          const uint64_t da0 = smem_desc_sw128(sQ, 16, 1024), db0 = smem_desc_sw128(sK, 16, 1024);
+          const uint64_t da0 = smem_desc_sw128(KV8 ? sQ8 : sQ, 16, 1024), db0 = smem_desc_sw128(sK, 16, 1024);
+          if constexpr (KV8) {
+            // e4m3: a 128-byte row holds all 128 channels; K = 32 channels = 32 bytes per instruction
 #pragma unroll
-          for (int kk = 0; kk < D / 16; ++kk)
-            mma_ss(tmem + (t & 1) * kSbCol, da0 + (uint64_t)(((kk >> 2) * L::kQChunk + (kk & 3) * 32) >> 4),
-                   db0 + (uint64_t)(((kk >> 2) * L::kKVChunk + (kk & 3) * 32) >> 4), idesc_qk, kk > 0);
+            for (int kk = 0; kk < D / 32; ++kk)
+              mma_ss_f8(tmem + (t & 1) * kSbCol, da0 + (uint64_t)((kk * 32) >> 4), db0 + (uint64_t)((kk * 32) >> 4), idesc_qk, kk > 0);
+          } else {
+#pragma unroll
+            for (int kk = 0; kk < D / 16; ++kk)
+              mma_ss(tmem + (t & 1) * kSbCol, da0 + (uint64_t)(((kk >> 2) * L::kQChunk + (kk & 3) * 32) >> 4),
+                     db0 + (uint64_t)(((kk >> 2) * L::kKVChunk + (kk & 3) * 32) >> 4), idesc_qk, kk > 0);
+          }
           mma_commit(bar(BAR_EMPTY + slot));
           mma_commit(bar(BAR_S_FULL + (t & 1)));
         }
         __syncwarp();
         ++c;
       };
-      mbar_wait(bar(BAR_Q_FULL), 0);
+      mbar_wait(bar(KV8 ? BAR_Q8 : BAR_Q_FULL), 0);
       issue_qk(0);
       if (Tn > 1) issue_qk(1);
       for (int t = 0; t < Tn; ++t) {
@@ -402,10 +417,18 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
         tc_fence_after();
         if (elect_one()) {
           const uint64_t db0 = smem_desc_sw128(sV, L::kKVChunk, 1024);
+          if constexpr (KV8) {
+            // P in e4m3: 32 keys = 8 TMEM columns per instruction; V rows (keys) of 128 bytes = all d channels, 32 rows on
 #pragma unroll
-          for (int kk = 0; kk < HALF / 16; ++kk)
-            mma_ts(tmem + kOCol, tmem + (t & 1) * kSbCol + kk * 8, db0 + (uint64_t)((kk * 2048) >> 4), idesc_pv,
-                   (t > 0 || kk > 0) ? 1u : 0u);
+            for (int kk = 0; kk < HALF / 32; ++kk)
+              mma_ts_f8(tmem + kOCol, tmem + (t & 1) * kSbCol + kk * 8, db0 + (uint64_t)((kk * 4096) >> 4), idesc_pv,
+                        (t > 0 || kk > 0) ? 1u : 0u);
+          } else {
+#pragma unroll
+            for (int kk = 0; kk < HALF / 16; ++kk)
+              mma_ts(tmem + kOCol, tmem + (t & 1) * kSbCol + kk * 8, db0 + (uint64_t)((kk * 2048) >> 4), idesc_pv,
+                     (t > 0 || kk > 0) ? 1u : 0u);
+          }
           mma_commit(bar(BAR_EMPTY + slot));
           mma_commit(bar(BAR_PV_DONE));
           if (t == Tn - 1) mma_commit(bar(BAR_O_FULL));
@@ -419,6 +442,49 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
       const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
       const int row = warp * 32 + lane;                // query row inside the tile == TMEM lane
       float m_used = 0.f, l = 0.f;
+      float scale_row = p.scale_log2;                  // logits (log2 units) per unit of the raw dot product S
+      if constexpr (KV8) {
+        // FP8 pages: both MMA operands are 8-bit, so the query row of this thread is replaced by its own e4m3 image:
+        // qs = max|q| / 448 (fp32; 1 for a zero row), code = e4m3(q / qs).  The bf16 row is read from the TMA-written
+        // tile (SWIZZLE_128B: 16-byte piece j of row r sits at piece j ^ (r mod 8)) and the codes are written in the
+        // same K-major swizzled layout, one 128-byte row per query.
+        mbar_wait(bar(BAR_Q_FULL), 0);
+        const uint8_t *qrow = smem + L::kOffQ + (row >> 3) * 1024 + (row & 7) * 128;
+        float amax = 0.f;
+#pragma unroll
+        for (int c = 0; c < D / 64; ++c)
+#pragma unroll
+          for (int jp = 0; jp < 8; ++jp) {
+            const uint4 v = *reinterpret_cast<const uint4 *>(qrow + c * L::kQChunk + ((jp ^ (row & 7)) << 4));
+            const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+            for (int e = 0; e < 4; ++e)
+              amax = fmaxf(amax, fmaxf(fabsf(__uint_as_float(w[e] << 16)), fabsf(__uint_as_float(w[e] & 0xffff0000u))));
+          }
+        const float qs = amax > 0.f ? __fdiv_rn(amax, 448.0f) : 1.0f;
+        uint8_t *q8row = smem + L::kOffQ8 + (row >> 3) * 1024 + (row & 7) * 128;
+#pragma unroll
+        for (int jo = 0; jo < 8; ++jo) {               // output piece jo = channels 16 jo .. 16 jo + 15 = two bf16 pieces
+          uint32_t out[4];
+#pragma unroll
+          for (int half_ = 0; half_ < 2; ++half_) {
+            const int ch = jo * 16 + half_ * 8, c = ch >> 6, jp = (ch & 63) >> 3;
+            const uint4 v = *reinterpret_cast<const uint4 *>(qrow + c * L::kQChunk + ((jp ^ (row & 7)) << 4));
+            const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+              const float x0 = __fdiv_rn(__uint_as_float(w[2 * e] << 16), qs), x1 = __fdiv_rn(__uint_as_float(w[2 * e] & 0xffff0000u), qs);
+              const float x2 = __fdiv_rn(__uint_as_float(w[2 * e + 1] << 16), qs), x3 = __fdiv_rn(__uint_as_float(w[2 * e + 1] & 0xffff0000u), qs);
+              out[half_ * 2 + e] = pack_e4m3x2(x0, x1) | (pack_e4m3x2(x2, x3) << 16);
+            }
+          }
+          *reinterpret_cast<uint4 *>(q8row + ((jo ^ (row & 7)) << 4)) = make_uint4(out[0], out[1], out[2], out[3]);
+        }
+        fence_proxy_async();                           // generic-proxy writes -> visible to the tensor core's smem reads
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar(BAR_Q8));
+        scale_row = p.scale_log2 * qs * __ldg(p.k_scale + h);   // S = (q / qs) . (k / ks): logits = S * qs * ks * scale
+      }
       int j = 0, hh = 0;
       if (SPLIT) {                                     // split query block: skip to this CTA's range
         for (int t = 0; t < t_lo; ++t) {
@@ -485,7 +551,7 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
           mx2 = fmaxf(mx2, __uint_as_float(s[c + 2]));
           mx3 = fmaxf(mx3, __uint_as_float(s[c + 3]));
         }
-        const float m_new = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * p.scale_log2;
+        const float m_new = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * scale_row;
 
         // lazy rescale: the reference maximum only moves when the row maximum grew by more than 2^8
         bool need = false;
@@ -510,7 +576,7 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
 
         // P = exp2(s*scale - m_used), row sum in fp32, bf16 pairs packed low = even column.  kEmuOf4 of every 4
         // column pairs take the FMA-pipe exp2 (li_ptx.cuh), the others the MUFU, so that both pipes stay busy.
-        const uint64_t sc2 = pack2(p.scale_log2, p.scale_log2), nm2 = pack2(-m_used, -m_used);
+        const uint64_t sc2 = pack2(scale_row, scale_row), nm2 = pack2(-m_used, -m_used);
         uint64_t sum_a = pack2(0.f, 0.f), sum_b = pack2(0.f, 0.f);
         uint32_t pk[HALF / 2];
 #pragma unroll
@@ -527,14 +593,20 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
           }
           if (c & 1) sum_b = add2(sum_b, pack2(p0, p1));
           else sum_a = add2(sum_a, pack2(p0, p1));
-          pk[c] = pack_bf16x2(p0, p1);
+          if constexpr (KV8) {                           // e4m3: four keys per 32-bit TMEM column, lowest key in the low byte
+            if (c & 1) pk[c >> 1] |= pack_e4m3x2(p0, p1) << 16;
+            else pk[c >> 1] = pack_e4m3x2(p0, p1);
+          } else {
+            pk[c] = pack_bf16x2(p0, p1);
+          }
         }
         {
           float a0, a1;
           unpack2(add2(sum_a, sum_b), a0, a1);
           l += a0 + a1;
         }
-        if constexpr (HALF == 64) tmem_st32(s_addr, *reinterpret_cast<uint32_t(*)[32]>(&pk[0]));
+        if constexpr (KV8) tmem_st16(s_addr, pk);      // 64 keys in e4m3 = 16 columns (FP8 pages: BLK == 128)
+        else if constexpr (HALF == 64) tmem_st32(s_addr, *reinterpret_cast<uint32_t(*)[32]>(&pk[0]));
         else tmem_st16(s_addr, pk);
         tc_wait_st();
         tc_fence_before();
@@ -554,6 +626,11 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
           uint32_t o[32];
           tmem_ld32(tmem + lane_base + kOCol + c * 32, o);
           tc_wait_ld();
+          if constexpr (KV8) {                           // O accumulates P . (v / vs): the per-head V scale goes in here
+            const float vs = __ldg(p.v_scale + h);
+#pragma unroll
+            for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * vs);
+          }
 #pragma unroll
           for (int e = 0; e < 32; e += 4)
             *reinterpret_cast<uint4 *>(po + c * 32 + e) = make_uint4(o[e], o[e + 1], o[e + 2], o[e + 3]);
@@ -561,7 +638,7 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
         p.part_ml[prow] = make_float2(m_used, l);
       } else {
         // epilogue: O / l -> bf16, stored in linear token order (no untile pass)
-        const float inv_l = 1.0f / l;
+        const float inv_l = (KV8 ? __ldg(p.v_scale + h) : 1.0f) / l;   // FP8 pages: O accumulated P . (v / vs)
         const int64_t u = row_token<BLK, K3D>(p, i, row);
         const bool live = u >= 0;
         uint16_t *orow = p.o + (((int64_t)b * p.H + h) * p.Lq + u) * D;
@@ -615,7 +692,16 @@ __global__ void __launch_bounds__(192, 2)
 li_sparse_attn_kernel(const AttnParams p, const BatchMeta meta, const __grid_constant__ CUtensorMap tm_q,
                       const __grid_constant__ CUtensorMap tm_k_full, const __grid_constant__ CUtensorMap tm_k_8,
                       const __grid_constant__ CUtensorMap tm_v_full, const __grid_constant__ CUtensorMap tm_v_8) {
-  attn_body<D, BLK, K3D, false, SPLIT>(p, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, tm_q, tm_q);
+  attn_body<D, BLK, K3D, false, SPLIT, false>(p, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, tm_q, tm_q);
+}
+
+// FP8 (E4M3) K/V pages: both contractions on the kind::f8f6f4 tensor-core path (d = 128, 128-token blocks)
+template <bool K3D, bool SPLIT>
+__global__ void __launch_bounds__(192, 2)
+li_sparse_attn_fp8_kernel(const AttnParams p, const BatchMeta meta, const __grid_constant__ CUtensorMap tm_q,
+                          const __grid_constant__ CUtensorMap tm_k_full, const __grid_constant__ CUtensorMap tm_k_8,
+                          const __grid_constant__ CUtensorMap tm_v_full, const __grid_constant__ CUtensorMap tm_v_8) {
+  attn_body<128, 128, K3D, false, SPLIT, true>(p, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, tm_q, tm_q);
 }
 
 template <int D, int BLK, bool K3D, bool SPLIT>
@@ -624,7 +710,7 @@ li_sparse_attn_text_kernel(const AttnParams p, const BatchMeta meta, const __gri
                            const __grid_constant__ CUtensorMap tm_k_full, const __grid_constant__ CUtensorMap tm_k_8,
                            const __grid_constant__ CUtensorMap tm_v_full, const __grid_constant__ CUtensorMap tm_v_8,
                            const __grid_constant__ CUtensorMap tm_tk, const __grid_constant__ CUtensorMap tm_tv) {
-  attn_body<D, BLK, K3D, true, SPLIT>(p, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, tm_tk, tm_tv);
+  attn_body<D, BLK, K3D, true, SPLIT, false>(p, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, tm_tk, tm_tv);
 }
 
 // Merges the n_split partial results of every split query block (tail-wave split): with reference maxima
@@ -666,12 +752,12 @@ __global__ void __launch_bounds__(256) li_attn_combine_kernel(const AttnParams p
     p.lse[((int64_t)b * p.H + h) * p.Lq + u] = L > 0.f ? (M + log2f(L)) * 0.6931471805599453f : __int_as_float(0xff800000);
 }
 
-template <int D, int BLK, bool K3D, bool TEXT, bool SPLIT>
+template <int D, int BLK, bool K3D, bool TEXT, bool SPLIT, bool KV8 = false>
 static int launch_one(const AttnParams &ap, const BatchMeta &meta, const CUtensorMap &tm_q, const CUtensorMap &tm_tk,
                       const CUtensorMap &tm_tv, const CUtensorMap &tm_k_full,
                       const CUtensorMap &tm_k_8, const CUtensorMap &tm_v_full, const CUtensorMap &tm_v_8,
                       cudaStream_t st) {
-  constexpr int smem = AttnSmem<D, BLK>::kTotal;
+  constexpr int smem = AttnSmem<D, BLK, KV8>::kTotal;
   cudaError_t e;
   // the dynamic shared-memory limit of this instance is raised once per device, not on every call
   static std::atomic<uint64_t> attr_done{0};
@@ -679,7 +765,8 @@ static int launch_one(const AttnParams &ap, const BatchMeta &meta, const CUtenso
   if ((e = cudaGetDevice(&dev)) != cudaSuccess) return (int)e;
   const uint64_t dev_bit = 1ull << (dev & 63);
   if (!(attr_done.load(std::memory_order_acquire) & dev_bit)) {
-    if constexpr (TEXT) e = cudaFuncSetAttribute(li_sparse_attn_text_kernel<D, BLK, K3D, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if constexpr (KV8) e = cudaFuncSetAttribute(li_sparse_attn_fp8_kernel<K3D, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    else if constexpr (TEXT) e = cudaFuncSetAttribute(li_sparse_attn_text_kernel<D, BLK, K3D, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     else e = cudaFuncSetAttribute(li_sparse_attn_kernel<D, BLK, K3D, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return (int)e;
     attr_done.fetch_or(dev_bit, std::memory_order_release);
@@ -695,7 +782,9 @@ static int launch_one(const AttnParams &ap, const BatchMeta &meta, const CUtenso
   cfg.stream = st;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  if constexpr (TEXT)
+  if constexpr (KV8)
+    e = cudaLaunchKernelEx(&cfg, li_sparse_attn_fp8_kernel<K3D, SPLIT>, ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8);
+  else if constexpr (TEXT)
     e = cudaLaunchKernelEx(&cfg, li_sparse_attn_text_kernel<D, BLK, K3D, SPLIT>, ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8, tm_tk, tm_tv);
   else
     e = cudaLaunchKernelEx(&cfg, li_sparse_attn_kernel<D, BLK, K3D, SPLIT>, ap, meta, tm_q, tm_k_full, tm_k_8, tm_v_full, tm_v_8);
@@ -748,11 +837,16 @@ int launch_attn(const AttnParams &ap_in, const BatchMeta &meta, int d, int blk, 
                   : launch_one<DD, BB, K3, TX, false>(ap, meta, tm_q, tm_tk, tm_tv, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st))
 #define LI_LAUNCH2(DD, BB, K3) (ap.Lt > 0 ? LI_LAUNCH3(DD, BB, K3, true) : LI_LAUNCH3(DD, BB, K3, false))
 #define LI_LAUNCH(DD, BB) (k3 ? LI_LAUNCH2(DD, BB, true) : LI_LAUNCH2(DD, BB, false))
-  if (d == 128 && blk == 128) e = LI_LAUNCH(128, 128);
+#define LI_LAUNCH_FP8(K3) \
+  (ap.n_split > 1 ? launch_one<128, 128, K3, false, true, true>(ap, meta, tm_q, tm_tk, tm_tv, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st) \
+                  : launch_one<128, 128, K3, false, false, true>(ap, meta, tm_q, tm_tk, tm_tv, tm_k_full, tm_k_8, tm_v_full, tm_v_8, st))
+  if (ap.k_scale != nullptr) e = k3 ? LI_LAUNCH_FP8(true) : LI_LAUNCH_FP8(false);   // FP8 pages: d = 128, block 128 (checked by the API)
+  else if (d == 128 && blk == 128) e = LI_LAUNCH(128, 128);
   else if (d == 128 && blk == 64) e = LI_LAUNCH(128, 64);
   else if (d == 64 && blk == 128) e = LI_LAUNCH(64, 128);
   else e = LI_LAUNCH(64, 64);
 #undef LI_LAUNCH
+#undef LI_LAUNCH_FP8
 #undef LI_LAUNCH2
 #undef LI_LAUNCH3
   if (e == 0 && n_launches) *n_launches += ap.n_split > 1 ? 2 : 1;

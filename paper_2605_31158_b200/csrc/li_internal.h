@@ -43,6 +43,7 @@ struct SelectParams {
   float *scores;   // optional
   float inv_sqrt_d;
   const float *slice_cache;   // 3-D tiling: per-page patch sums [n_pages,H,Hb*Wb,d]; non-null: kbar is formed from them
+  const float *k_scale;       // LI_FLAG_KV_FP8: k_cache holds e4m3 codes (byte strides), value = decode * k_scale[h]
 };
 
 struct AttnParams {
@@ -57,6 +58,7 @@ struct AttnParams {
   const int32_t *sel_cnt;
   uint16_t *o;
   float *lse;
+  const float *k_scale, *v_scale;   // LI_FLAG_KV_FP8: per-head scales of the e4m3 K / V pages (else null)
   // tail-wave split: CTAs [0, split_first) own a whole query block each; from split_first on, n_split
   // consecutive CTAs share one query block, each taking a contiguous range of its half-tiles and writing unnormalised
   // partial results, which li_attn_combine_kernel merges.  n_split == 1: no split (split_first == number of blocks).
@@ -69,6 +71,17 @@ constexpr int kMaxSplitSlots = 320;   // upper bound of split CTAs (<= 2 CTAs pe
 
 // launches (defined in the .cu files); return cudaError_t as int
 int launch_select(const SelectParams &sp, const BatchMeta &meta, cudaStream_t st, int64_t *n_launches);
+// FP8 pages (li_fp8.cu): pooling of the historical K blocks from e4m3 pages; quantise-on-write
+int launch_pool_k8(const SelectParams &sp, const BatchMeta &meta, cudaStream_t st, int64_t *n_launches);
+struct QuantParams {
+  int32_t H, T_f, d, n_pages;
+  const uint16_t *k_src, *v_src;      // bf16 [n_list,H,T_f,d]
+  uint8_t *k_cache, *v_cache;
+  int64_t kv_sp, kv_sh, kv_st;
+  const float *k_scale, *v_scale;
+  const int32_t *pages;
+};
+int launch_quantize_pages(const QuantParams &qp, int n_list, cudaStream_t st, int64_t *n_launches);
 int launch_pool_pages(const SelectParams &sp, const int32_t *pages, int n_list, float *cache, cudaStream_t st, int64_t *n_launches);
 int launch_attn(const AttnParams &ap, const BatchMeta &meta, int d, int blk, const CUtensorMap &tm_q,
                 const CUtensorMap &tm_tk, const CUtensorMap &tm_tv, const CUtensorMap &tm_k_full, const CUtensorMap &tm_k_8, const CUtensorMap &tm_v_full,

@@ -513,7 +513,9 @@ static cudaError_t launch_score_topk(cudaLaunchConfig_t &cfg, const SelectParams
 
 int launch_select(const SelectParams &sp, const BatchMeta &meta, cudaStream_t st, int64_t *n_launches) {
   {
-    dim3 grid(sp.Nqb + (sp.skip_k ? 0 : sp.Mmax), sp.H, sp.B);
+    // FP8 pages: the bf16 pool kernel takes the query blocks only, li_pool_k8_kernel the historical K blocks
+    const bool k8 = sp.k_scale != nullptr;
+    dim3 grid(sp.Nqb + ((sp.skip_k || k8) ? 0 : sp.Mmax), sp.H, sp.B);
     if (sp.tl.bt > 0) {
       if (sp.d == 128) li_pool_kernel<128, true><<<grid, kPoolThreads, 0, st>>>(sp, meta);
       else li_pool_kernel<64, true><<<grid, kPoolThreads, 0, st>>>(sp, meta);
@@ -524,6 +526,10 @@ int launch_select(const SelectParams &sp, const BatchMeta &meta, cudaStream_t st
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return (int)e;
     if (n_launches) *n_launches += 1;
+    if (k8 && !sp.skip_k) {
+      const int e8 = launch_pool_k8(sp, meta, st, n_launches);
+      if (e8 != 0) return e8;
+    }
   }
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
