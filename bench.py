@@ -237,7 +237,16 @@ def run_cuda(args):
     buf = li.Buffers(ctx, prob.kmax, want_scores=False, want_lse=True)
     o_host = torch.empty(buf.o.shape, dtype=buf.o.dtype).pin_memory()
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)   # > 126 MB L2
+    flush_words = flush.view(torch.int64)[::16]                            # one 8-byte word of every 128-byte line
     stream = torch.cuda.current_stream()
+
+    def flush_l2(tag: int):
+        """Between timed steps: WRITE a buffer twice the size of the L2 (evicts every line of the workload), then READ one
+        word of each of its lines, so that the dirty lines the write left behind are written back now and not under the
+        first kernel of the next step (the HBM-bound pool kernel would otherwise share the bus with ~126 MB of
+        write-backs).  Both passes run outside the CUDA events."""
+        flush.fill_(tag & 0xff)
+        flush_words.sum()
 
     def step(ev=None):
         if ev is not None:
@@ -318,7 +327,7 @@ def run_cuda(args):
         torch.cuda.synchronize()
 
     for _ in range(max(3, args.warmup)):
-        flush.fill_(1)
+        flush_l2(1)
         step()
     torch.cuda.synchronize()
     sel_idx = buf.sel_idx.cpu().numpy()
@@ -332,7 +341,7 @@ def run_cuda(args):
     with ClockSampler(local) as clk:
         t_wall0 = time.perf_counter()
         for k in range(args.steps):
-            flush.fill_(k & 0xff)
+            flush_l2(k & 0xff)
             step(evs[k])
         barrier()
         launches = li.launch_count()            # counted by the library inside the timed region
@@ -377,11 +386,11 @@ def run_cuda(args):
     #      pool minus attention over the same context laid out contiguously with an identity frame list ----
     extras = {}
     if world == 1 and not args.no_extras:
-        def time_attn(cx, n=10, flush_l2=True):
+        def time_attn(cx, n=10, cold=True):
             ts = []
             for _ in range(n):
-                if flush_l2:
-                    flush.fill_(3)
+                if cold:
+                    flush_l2(3)
                 a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 a.record(stream)
                 li.li_sparse_attn(cx, buf.sel_idx, buf.sel_cnt, buf.kmax, buf.o, buf.lse, buf.workspace, stream)
@@ -389,10 +398,10 @@ def run_cuda(args):
                 torch.cuda.synchronize()
                 ts.append(a.elapsed_time(b_))
             return float(np.mean(ts[2:]))
-        extras["attn_ms_l2_warm"] = time_attn(ctx, flush_l2=False)
+        extras["attn_ms_l2_warm"] = time_attn(ctx, cold=False)
         ts = []
         for _ in range(12):                              # select with the pooled history keys reused (denoising steps 2..K)
-            flush.fill_(5)
+            flush_l2(5)
             a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a.record(stream)
             li.li_block_select(ctx, prob.top_k, buf.kmax, buf.sel_idx, buf.sel_cnt, buf.workspace, None, stream, reuse_kbar=True)
@@ -408,7 +417,7 @@ def run_cuda(args):
             cur_t = torch.tensor(cur_pages, dtype=torch.int32, device=dev)
             t_sel, t_pool = [], []
             for _ in range(12):
-                flush.fill_(6)
+                flush_l2(6)
                 a, b_, c_ = (torch.cuda.Event(enable_timing=True) for _ in range(3))
                 a.record(stream)
                 li.li_pool_pages(ctx, cur_t, cache, stream)
@@ -446,7 +455,7 @@ def run_cuda(args):
             sp = torch.rand(8, device=dev)
             ts = []
             for _ in range(reps):
-                flush.fill_(7)
+                flush_l2(7)
                 a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 a.record(stream)
                 li.li_context_policy(z1, z2, ema, 0.3, 0.02, 16, sp, 0.45, pages[:4], pages[4:24], pages[24:28], out, res, ws,
@@ -490,7 +499,7 @@ def run_cuda(args):
             "config": {"workload": s.name, "B": prob.B, "H": s.H, "d": s.d, "Lq": prob.Lq, "frame_tokens": s.frame_tokens,
                        "block": s.block, "block3d": s.block3d, "grid": s.grid, "kv": args.kv, "Lk": [prob.L_hist(b) + prob.Lq for b in range(prob.B)],
                        "top_k": [int(x) for x in prob.top_k], "M": [prob.M(b) for b in range(prob.B)],
-                       "l2": "flushed between timed steps (256 MiB write)", "multi_gpu": "replicas only (no collective)"},
+                       "l2": "flushed between timed steps (256 MiB written, then read back so that no dirty line is left)", "multi_gpu": "replicas only (no collective)"},
             "effective_flops_per_step": int(flops),
             "select_ms": float(sel_ms.mean()), "attn_ms": float(att_ms.mean()), "attn_ms_min": float(att_ms.min()),
             "select_overhead_frac_of_attn": float(sel_ms.mean() / att_ms.mean()),

@@ -513,7 +513,6 @@ __device__ __forceinline__ void attn_body(const AttnParams &p, const BatchMeta &
         bool rows_full = true;
 #pragma unroll
         for (int s_ = 0; s_ < SPH; ++s_) rows_full = rows_full && vs[s_] == 32;
-        const bool full = rows_full && vw == 0;
         if (hh == 0 && halves(j) > 1) hh = 1;
         else { ++j; hh = 0; }
         const uint32_t s_addr = tmem + lane_base + (t & 1) * kSbCol;
