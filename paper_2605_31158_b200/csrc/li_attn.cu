@@ -16,7 +16,11 @@
 // TMEM (256 columns): [0,HALF) S_a, [64,64+HALF) S_b (fp32; P in bf16 overlays the first HALF/2 columns of its S
 // buffer once S has been read), [128,128+D) O.
 // On B200 this kernel runs into the 1 kW power cap (SM clock ~1.6 GHz under load); DESIGN.md section 6.3 lists the
-// measured alternatives (one CTA per SM with Q in tensor memory, two softmax groups, FMA-pipe exp2, ...).
+// measured alternatives (one CTA per SM with Q in tensor memory, two softmax groups, FMA-pipe exp2, full-tile QK,
+// speculative / prefetching softmax loop, ...).
+// KV8 instances (LI_FLAG_KV_FP8): K/V pages hold e4m3 codes; the softmax warps first turn the bf16 Q
+// tile into its per-row e4m3 image in shared memory, both contractions run on tcgen05.mma.kind::f8f6f4 and P is
+// rounded to e4m3 (four keys per TMEM column).
 #include <atomic>
 
 #include "li_internal.h"

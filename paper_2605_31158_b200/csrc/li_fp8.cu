@@ -78,7 +78,10 @@ __global__ void __launch_bounds__(256, 4) li_pool_k8_kernel(const SelectParams p
   const int n_hist = meta.frame_off[b + 1] - foff - p.n_cur;
   const int32_t *pages = p.frame_idx + foff;
   const Tiling tl = p.tl;
-  if (m >= tl.num_blocks(n_hist, p.T_f, p.blk)) return;
+  if (m >= tl.num_blocks(n_hist, p.T_f, p.blk)) {
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    return;
+  }
   const uint8_t *base = reinterpret_cast<const uint8_t *>(p.k_cache) + h * p.kv_sh + cofs;
   auto page_base = [&](int f) -> const uint8_t * {
     const int pg = __ldg(pages + f);
@@ -102,14 +105,28 @@ __global__ void __launch_bounds__(256, 4) li_pool_k8_kernel(const SelectParams p
   } else {
     const int L = n_hist * p.T_f, t0 = m * p.blk;
     nvalid = min(p.blk, L - t0);
+    if (p.T_f >= p.blk) {
+      // the block touches at most two pages: rows [0, split) lie in page F[pg0], the rest in page F[pg0 + 1]
+      const int pg0 = t0 / p.T_f, row0 = t0 - pg0 * p.T_f, split = p.T_f - row0;
+      const uint8_t *b0 = page_base(pg0), *b1 = split < nvalid ? page_base(pg0 + 1) : nullptr;
+      if (b0 != nullptr) b0 += (int64_t)row0 * p.kv_st;
+      if (b1 != nullptr) b1 -= (int64_t)split * p.kv_st;
 #pragma unroll
-    for (int it = 0; it < kIter; ++it) {
-      const int r = r0 + it * RPP;
-      v[it] = make_uint4(0, 0, 0, 0);
-      if (r < nvalid) {
-        const int t = t0 + r, pg = t / p.T_f;
-        const uint8_t *rb = page_base(pg);
-        if (rb != nullptr) v[it] = ldg_stream16(rb + (int64_t)(t - pg * p.T_f) * p.kv_st);
+      for (int it = 0; it < kIter; ++it) {
+        const int r = r0 + it * RPP;
+        const uint8_t *rb = r < split ? b0 : b1;
+        v[it] = (r < nvalid && rb != nullptr) ? ldg_stream16(rb + (int64_t)r * p.kv_st) : make_uint4(0, 0, 0, 0);
+      }
+    } else {
+#pragma unroll
+      for (int it = 0; it < kIter; ++it) {               // frames shorter than a block: one page lookup per row
+        const int r = r0 + it * RPP;
+        v[it] = make_uint4(0, 0, 0, 0);
+        if (r < nvalid) {
+          const int t = t0 + r, pg = t / p.T_f;
+          const uint8_t *rb = page_base(pg);
+          if (rb != nullptr) v[it] = ldg_stream16(rb + (int64_t)(t - pg * p.T_f) * p.kv_st);
+        }
       }
     }
   }
@@ -137,15 +154,27 @@ __global__ void __launch_bounds__(256, 4) li_pool_k8_kernel(const SelectParams p
     for (int r = 0; r < RPP; ++r) s += red[r][threadIdx.x];
     p.kbar[(((int64_t)b * p.H + h) * D + threadIdx.x) * p.Mp + m] = __ldg(p.k_scale + h) * (s / (float)nvalid);
   }
+  // launched as a programmatic dependent of the bf16 pool kernel (query blocks), with which it shares nothing: the two
+  // overlap; waiting here, after the work, makes this grid's completion imply that one's for the kernels that follow
+  asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
 int launch_pool_k8(const SelectParams &sp, const BatchMeta &meta, cudaStream_t st, int64_t *n_launches) {
   if (sp.Mmax <= 0) return 0;
-  dim3 grid(sp.Mmax, sp.H, sp.B);
-  if (sp.tl.bt > 0) li_pool_k8_kernel<true><<<grid, 256, 0, st>>>(sp, meta);
-  else li_pool_k8_kernel<false><<<grid, 256, 0, st>>>(sp, meta);
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(sp.Mmax, sp.H, sp.B);
+  cfg.blockDim = dim3(256);
+  cfg.stream = st;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  const cudaError_t e = sp.tl.bt > 0 ? cudaLaunchKernelEx(&cfg, li_pool_k8_kernel<true>, sp, meta)
+                                      : cudaLaunchKernelEx(&cfg, li_pool_k8_kernel<false>, sp, meta);
+  if (e != cudaSuccess) return (int)e;
   if (n_launches) *n_launches += 1;
-  return (int)cudaGetLastError();
+  return 0;
 }
 
 }  // namespace li

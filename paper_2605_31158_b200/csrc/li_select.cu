@@ -2,9 +2,11 @@
 //   kernel 1  li_pool_kernel        : block means of Q and of the historical K (K rows fetched through the
 //                                     frame-index list, in place).  HBM-bound streaming reduction: every Q and
 //                                     historical-K byte is read exactly once with 16-byte loads.
-//   kernel 2  li_score_topk_kernel  : one warp per (call, head, query block) row: scores qbar_i . kbar_m / sqrt(d)
-//                                     (fp32) stay in registers as order-preserving keys, an MSB-first radix select
-//                                     finds the k-th largest, ties -> lowest block index, indices written ascending.
+//   kernel 2  li_score_topk_kernel  : one CTA per 16 query-block rows of a (call, head): kbar streamed into shared memory
+//                                     by bulk async copies, scores qbar_i . kbar_m / sqrt(d) (fp32, packed FMAs), then
+//                                     one warp per row: the scores stay in registers as order-preserving keys, an
+//                                     MSB-first radix select finds the k-th largest, ties -> lowest block index,
+//                                     indices written ascending.
 //   (M > 512 historical blocks: li_score_kernel writes the keys to the workspace and li_topk_kernel selects from there.)
 #include <atomic>
 

@@ -104,6 +104,13 @@ def test_fp8_pages_3d_blocks_and_split(env):
     assert li.lib().li_launch_count() == 1 + 5      # quantise | Q pool, K pool (fp8), score + top-k, attention (split), merge
 
 
+def test_fp8_pages_right_border_blocks(env):
+    """(4,4,8) blocks on a grid whose width is not a multiple of 8: column-masked border tiles with e4m3 pages."""
+    spec = W.spec_small(name="fp8-3d-448", H=2, d=128, block=128, frame_tokens=10 * 12, n_cur_frames=4, n_pages=14, n_mem=(2,),
+                        n_win=(3,), density=Fraction(1, 2), grid=(10, 12), block3d=(4, 4, 8))
+    run_case(env, spec)
+
+
 def test_fp8_varlen_batch_and_growing_maximum(env):
     """Several calls of different length in one launch; later pages up to 4.6x louder, so the lazy rescale path runs with
     e4m3 P.  The louder keys make the softmax rows peaky (a handful of keys carry a row), where the rounding of P no
