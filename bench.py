@@ -481,6 +481,27 @@ def run_cuda(args):
         torch.cuda.synchronize()
         extras["step_ms_sustained"] = a.elapsed_time(b_) / n_sus
         extras["step_ms_sustained_note"] = f"{n_sus} back-to-back steps after {n_sus // 3} untimed ones, no L2 flush"
+        if s.name == "dense-equivalence":
+            # BASELINE.json configs[4], second half: li_block_select ALONE on the `long` shapes (Lk = 56160), timed as an
+            # HBM-bound kernel: algorithmic bytes (Lq + L_hist) * d * 2 * H over its CUDA-event time, against the copy peak
+            lprob = W.build(W.spec_by_name("long"))
+            ls = lprob.spec
+            lctx = li.Context(lprob.q.to(dev), lprob.k_cache.to(dev), lprob.v_cache.to(dev), torch.from_numpy(lprob.frame_idx).to(dev),
+                              lprob.frame_off, ls.n_cur_frames, ls.block)
+            lbuf = li.Buffers(lctx, lprob.kmax, want_scores=False, want_lse=False)
+            ts = []
+            for _ in range(14):
+                flush_l2(9)
+                a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                li.li_block_select(lctx, lprob.top_k, lbuf.kmax, lbuf.sel_idx, lbuf.sel_cnt, lbuf.workspace, None, stream)
+                b_.record(stream)
+                torch.cuda.synchronize()
+                ts.append(a.elapsed_time(b_))
+            lbytes = (lprob.Lq + lprob.L_hist(0)) * ls.d * 2 * ls.H
+            t_sel = float(np.mean(ts[2:]))
+            extras["block_select_alone_long"] = {"ms": t_sel, "bytes": int(lbytes), "gbs": lbytes / (t_sel * 1e-3) / 1e9,
+                                                 "frac_of_hbm_peak": lbytes / (t_sel * 1e-3) / 1e9 / peaks()["hbm_gbs"], "Lk": lprob.L_hist(0) + lprob.Lq}
 
     total_ms, e2e_ms = max_over_ranks([total_ms, e2e_ms], dev, world)
     if rank == 0:

@@ -271,7 +271,7 @@ static int block_select_impl(const li_problem *p, const int32_t *top_k_host, int
 
 size_t li_slice_cache_bytes(const li_problem *p) {
   Derived dv;
-  if (check_problem(p, &dv, true) != LI_OK) return 0;
+  if (check_problem(p, &dv, true) != LI_OK || (p->flags & LI_FLAG_KV_FP8)) return 0;   // bf16 pages only
   return (size_t)p->n_pages * p->H * dv.tl.Hb * dv.tl.Wb * p->d * 4;
 }
 

@@ -254,3 +254,34 @@ def test_no_device_means_cuda_error_not_a_fallback(L):
     ws = L.li_workspace_bytes(ctypes.byref(p), 8)
     assert L.li_block_select(ctypes.byref(p), tk.ctypes.data, 8, 0x60000, 0x70000, None, 0, 0x50000, ws, None) == li.LI_ERR_CUDA
     assert L.li_last_cuda_error() != 0
+
+
+def test_fp8_pages_argument_checks(L):
+    """LI_FLAG_KV_FP8 (include/li.h): d = 128 and 128-token blocks only, scales required, byte strides multiples of 16, no text
+    prefix, no page-resident patch sums; li_quantize_pages host-side rejections."""
+    fo = np.asarray([0, 6], dtype=np.int32)
+
+    def prob8(**over):
+        p, _ = make_problem(frame_tokens=1560, Lq=2 * 1560, d=128, block_q=128, block_k=128, n_cur_frames=2, H=24,
+                            q_sb=24 * 3120 * 128, q_sh=3120 * 128, q_st=128, kv_sp=24 * 1560 * 128, kv_sh=1560 * 128, kv_st=128,
+                            flags=li.LI_FLAG_KV_FP8, k_scale=0xB0000, v_scale=0xC0000)
+        p.frame_off_host = fo.ctypes.data
+        for k, v in over.items():
+            setattr(p, k, v)
+        return p
+
+    assert L.li_workspace_bytes(ctypes.byref(prob8()), 8) > 0
+    for bad in (dict(d=64, q_st=64, kv_st=64), dict(block_q=64, block_k=64), dict(k_scale=0), dict(v_scale=0), dict(kv_st=136),
+                dict(Lt=16, text_k=0x90000, text_v=0xA0000, t_sb=24 * 16 * 128, t_sh=16 * 128, t_st=128)):
+        assert L.li_workspace_bytes(ctypes.byref(prob8(**bad)), 8) == 0, bad
+    p3 = prob8(grid_h=30, grid_w=52, bt=4, bh=8, bw=4)
+    assert L.li_workspace_bytes(ctypes.byref(p3), 8) > 0                   # 3-D blocks are supported with FP8 pages
+    assert L.li_slice_cache_bytes(ctypes.byref(p3)) == 0                   # ... page-resident patch sums are not
+    assert L.li_pool_pages(ctypes.byref(p3), 0x50000, 1, 0x60000, None) == li.LI_ERR_UNSUPPORTED
+    p = prob8()
+    q = lambda prob, ks=0x100000, vs=0x200000, pages=0x50000, n=2: L.li_quantize_pages(ctypes.byref(prob), ks, vs, pages, n, None)
+    assert q(p, n=0) == li.LI_OK                                           # nothing to do
+    assert q(p, ks=0) == li.LI_ERR_INVALID_ARG and q(p, pages=0) == li.LI_ERR_INVALID_ARG and q(p, n=-1) == li.LI_ERR_INVALID_ARG
+    assert q(p, vs=0x200008) == li.LI_ERR_INVALID_ARG                      # 16-byte alignment
+    assert q(prob8(flags=0)) == li.LI_ERR_INVALID_ARG                      # the problem does not describe FP8 pages
+    assert q(prob8(d=64, q_st=64, kv_st=64)) == li.LI_ERR_UNSUPPORTED
