@@ -828,7 +828,10 @@ int launch_attn(const AttnParams &ap_in, const BatchMeta &meta, int d, int blk, 
       const int t_est = 2 * ((ap.Lt + blk - 1) / blk + ap.Nc + ap.kmax);   // half-tiles per query block, upper bound
       int s = slots / rem;
       if (s > 8) s = 8;
-      if (s > t_est / 16) s = t_est / 16;               // at least ~16 half-tiles per CTA
+      // at least ~16 half-tiles per CTA in a tail wave; a grid that fills less than one wave is pure latency, there 6
+      // half-tiles per CTA still pay for the merge (`tiny`: 26.2 -> 18.0 us, thresholds 16 / 8 / 6 / 4 measured)
+      const int min_ht = n_work < wave ? 6 : 16;
+      if (s > t_est / min_ht) s = t_est / min_ht;
       if (s >= 2) {
         ap.n_split = s;
         ap.split_first = n_work - rem;
