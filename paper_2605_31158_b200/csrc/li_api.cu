@@ -9,6 +9,18 @@
 
 #include "li_internal.h"
 
+namespace li {
+int device_sm_count() {
+  static std::atomic<int> sm_count[64];
+  int dev = 0, n_sm = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return 0;
+  n_sm = sm_count[dev & 63].load(std::memory_order_relaxed);
+  if (n_sm == 0 && cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess)
+    sm_count[dev & 63].store(n_sm, std::memory_order_relaxed);
+  return n_sm;
+}
+}  // namespace li
+
 namespace {
 
 std::atomic<int64_t> g_launches{0};

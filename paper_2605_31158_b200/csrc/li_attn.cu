@@ -814,13 +814,7 @@ int launch_attn(const AttnParams &ap_in, const BatchMeta &meta, int d, int blk, 
   const int n_work = ap.Nqb * ap.H * ap.B;
   ap.split_first = n_work;
   ap.n_split = 1;
-  static std::atomic<int> sm_count[64];                  // multiprocessors per device, queried once
-  int dev = 0, n_sm = 0;
-  if (ap.part_o != nullptr && !ap.no_split && cudaGetDevice(&dev) == cudaSuccess) {
-    n_sm = sm_count[dev & 63].load(std::memory_order_relaxed);
-    if (n_sm == 0 && cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess)
-      sm_count[dev & 63].store(n_sm, std::memory_order_relaxed);
-  }
+  const int n_sm = (ap.part_o != nullptr && !ap.no_split) ? device_sm_count() : 0;
   if (n_sm > 0) {
     const int wave = 2 * n_sm, slots = wave < kMaxSplitSlots ? wave : kMaxSplitSlots;
     const int rem = n_work % wave;

@@ -69,6 +69,9 @@ struct AttnParams {
 
 constexpr int kMaxSplitSlots = 320;   // upper bound of split CTAs (<= 2 CTAs per SM), sizes the workspace
 
+// multiprocessors of the current device, queried once per device (0 if the query fails); defined in li_api.cu
+int device_sm_count();
+
 // launches (defined in the .cu files); return cudaError_t as int
 int launch_select(const SelectParams &sp, const BatchMeta &meta, cudaStream_t st, int64_t *n_launches);
 // FP8 pages (li_fp8.cu): pooling of the historical K blocks from e4m3 pages; quantise-on-write

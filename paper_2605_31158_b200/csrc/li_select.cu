@@ -158,35 +158,76 @@ __device__ __forceinline__ uint32_t order_key(float s) {
 }
 
 // ----------------------------------------------------------------------------- fused scores + Top_k (Eq. 10), M <= 512
-// One CTA = up to 16 consecutive query-block rows of one (call, head); grid = (ceil(Nqb / rows), B*H), 16 warps.
+// One CTA = up to 16 consecutive query-block rows of one (call, head); grid = (ceil(Nqb / rows), B*H), 16 warps; rows per
+// CTA are chosen on the host so that the grid fills, but stays inside, one wave of one CTA per SM where it can.
 // The head's pooled keys kbar[bh] (channel-major [D][Mp], contiguous) are streamed into shared memory by bulk async
 // copies (cp.async.bulk + mbarrier), one per channel quarter, all issued up front (fewer when four do not fit; the
 // others follow into the slots read first): no load latency is paid per FMA and no register holds data in flight.
-// Phase 1 (scores): warp w = (32-block group g = w mod nxp, channel part cp = w / nxp) holds ALL 16 rows against the 32
-//   blocks m = 32 g + lane (nxp = Mp / 32 groups): per channel one conflict-free LDS of kbar, four broadcast LDS.128 of the 16 pooled query
-//   values and 8 packed FMAs (fma.rn.f32x2: two rows per instruction).  The 16 / nxp channel parts take interleaved
-//   channels; their partial sums go to shared memory [part][row][Mp].
+// Phase 1 (scores): warp w = (32-block group g = w mod nxp, channel part cp = w / nxp) holds all rows of the CTA, by
+//   quads, against the 32 blocks m = 32 g + lane (nxp = Mp / 32 groups): per channel one conflict-free LDS of kbar, one
+//   broadcast LDS.128 of pooled query values and 2 packed FMAs (fma.rn.f32x2: two rows per instruction) per row quad in
+//   use (the loop is instantiated for 1..4 quads; addresses advance by constant steps).  The 16 / nxp channel parts take
+//   interleaved channels; their partial sums go to shared memory [part][row][Mp].
 // Phase 2 (Top_k): warp w owns row w: a score is the sum of its parts in a fixed order; the scores stay in registers as
-//   order-preserving keys, the k-th largest is found by an MSB-first radix select (32 counting passes with
-//   redux.sync), and one ordered pass emits, ascending, every block above the threshold plus the lowest-index blocks
-//   equal to it.
+//   order-preserving keys, the k-th largest is found by an MSB-first radix select (one counting pass with redux.sync per
+//   bit, ending early once exactly k keys pass), and one ordered pass emits, ascending, every block above the threshold
+//   plus the lowest-index blocks equal to it.
 constexpr int kSelWarps = 16;
 constexpr int kSelRowsMax = 16;
 constexpr int kSelPartFloats = kSelRowsMax * 16 * 32;      // [parts][16 rows][Mp] with parts * Mp <= 16 * 32
 __host__ __device__ inline size_t sel_smem_bytes(int D, int Mp, int n_slots) {
   return 128 + (size_t)(D * kSelRowsMax + kSelPartFloats + n_slots * (D / 4) * Mp) * sizeof(float);
 }
-// pooled query value (channel c, row r) lives at float c*16 + 4*((r/4) ^ (c & 3)) + r%4: a warp reads 4 consecutive rows
-// with one broadcast LDS.128 (the XOR permutes whole row quads) and the channel-major staging stores of consecutive
-// channels spread over the banks
-__device__ __forceinline__ int sq_index(int c, int r) { return c * kSelRowsMax + ((((r >> 2) ^ (c & 3)) << 2) | (r & 3)); }
+// pooled query value (channel c, row r) lives at float c*16 + r: a warp reads 4 consecutive rows with one broadcast
+// LDS.128; staged by one STS.128 per (channel, row quad)
+// One channel quarter of phase 1 for a warp: channels c = cp, cp + parts, ... of the quarter, RQ row quads (4 RQ rows)
+// against the 32 blocks of the warp's group; unrolled by 4 channels with the kbar loads up front.
+template <int RQ>
+__device__ __forceinline__ void score_quarter(const float *kq, const float *qq, int cp, int parts, int DW, int Mp,
+                                              uint64_t (&acc)[kSelRowsMax / 2]) {
+  const int kstep = parts * Mp, qstep = parts * kSelRowsMax;
+  kq += (size_t)cp * Mp;
+  qq += cp * kSelRowsMax;
+  int c = cp;
+  for (; c + 3 * parts < DW; c += 4 * parts) {
+    float kv[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) kv[u] = kq[u * kstep];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const uint64_t kk = pack2(kv[u], kv[u]);
+#pragma unroll
+      for (int rq = 0; rq < RQ; ++rq) {
+        const float4 q4 = *reinterpret_cast<const float4 *>(qq + u * qstep + 4 * rq);
+        acc[2 * rq] = fma2(pack2(q4.x, q4.y), kk, acc[2 * rq]);
+        acc[2 * rq + 1] = fma2(pack2(q4.z, q4.w), kk, acc[2 * rq + 1]);
+      }
+    }
+    kq += 4 * kstep;
+    qq += 4 * qstep;
+  }
+  for (; c < DW; c += parts) {
+    const float kv = *kq;
+    const uint64_t kk = pack2(kv, kv);
+#pragma unroll
+    for (int rq = 0; rq < RQ; ++rq) {
+      const float4 q4 = *reinterpret_cast<const float4 *>(qq + 4 * rq);
+      acc[2 * rq] = fma2(pack2(q4.x, q4.y), kk, acc[2 * rq]);
+      acc[2 * rq + 1] = fma2(pack2(q4.z, q4.w), kk, acc[2 * rq + 1]);
+    }
+    kq += kstep;
+    qq += qstep;
+  }
+}
 
-template <int D, int NX>
-__global__ void __launch_bounds__(kSelWarps * 32) li_score_topk_kernel(const SelectParams p, const BatchMeta meta,
+// MINB = 1: register budget of one CTA per SM (all loads of four channels in flight), for grids inside one wave;
+// MINB = 2: 64 registers, two CTAs per SM where the shared memory allows it (many calls x heads).
+template <int D, int NX, int MINB>
+__global__ void __launch_bounds__(kSelWarps * 32, MINB) li_score_topk_kernel(const SelectParams p, const BatchMeta meta,
                                                                         const int rows_per_cta, const int n_slots) {
   extern __shared__ __align__(128) uint8_t sel_smem[];
   constexpr int DW = D / 4;
-  float *sqT = reinterpret_cast<float *>(sel_smem + 128);  // [D][16], see sq_index
+  float *sqT = reinterpret_cast<float *>(sel_smem + 128);  // [D][16 rows]
   float *part = sqT + D * kSelRowsMax;                     // [parts][16][Mp]: partial dot products
   float *ring = part + kSelPartFloats;                     // [n_slots][DW][Mp]: channel quarters of kbar[bh]
   const uint32_t bar0 = smem_u32(sel_smem);                // 4 mbarriers, one per channel quarter (each used once)
@@ -218,12 +259,19 @@ __global__ void __launch_bounds__(kSelWarps * 32) li_score_topk_kernel(const Sel
   if (scoring) {
     if (threadIdx.x == 0)
       for (int q = 0; q < n_slots; ++q) copy_quarter(q);
-    for (int t = threadIdx.x; t < kSelRowsMax * D; t += kSelWarps * 32) {
-      const int r = t / D, c = t - r * D;
-      sqT[sq_index(c, r)] = r < R ? __ldg(p.qbar + ((int64_t)bh * p.Nqb + i0 + r) * D + c) : 0.f;
+    for (int t = threadIdx.x; t < (kSelRowsMax / 4) * D; t += kSelWarps * 32) {
+      const int rq = t / D, c = t - rq * D;                // consecutive lanes: consecutive channels (coalesced loads)
+      const float *src = p.qbar + ((int64_t)bh * p.Nqb + i0 + 4 * rq) * D + c;
+      float4 v;
+      v.x = 4 * rq + 0 < R ? __ldg(src) : 0.f;
+      v.y = 4 * rq + 1 < R ? __ldg(src + D) : 0.f;
+      v.z = 4 * rq + 2 < R ? __ldg(src + 2 * D) : 0.f;
+      v.w = 4 * rq + 3 < R ? __ldg(src + 3 * D) : 0.f;
+      *reinterpret_cast<float4 *>(sqT + c * kSelRowsMax + 4 * rq) = v;
     }
     __syncthreads();                                       // barriers initialised, query values staged
     const int g = warp % nxp, cp = warp / nxp;             // idle: cp >= parts (16 is not a multiple of nxp), g >= nx (short call)
+    const int nrq = (rows_per_cta + 3) >> 2;               // row quads held by a CTA of this launch (1..4)
     uint64_t acc[kSelRowsMax / 2];                         // acc[rp] = (row 2 rp, row 2 rp + 1) against block 32 g + lane
 #pragma unroll
     for (int rp = 0; rp < kSelRowsMax / 2; ++rp) acc[rp] = 0ull;
@@ -232,33 +280,11 @@ __global__ void __launch_bounds__(kSelWarps * 32) li_score_topk_kernel(const Sel
       if (cp < parts && g < nx) {
         const float *kq = ring + (size_t)(q % n_slots) * DW * p.Mp + 32 * g + lane;
         const float *qq = sqT + (size_t)q * DW * kSelRowsMax;
-        // this part's channels of the quarter: c = cp, cp + parts, ...; unrolled by 4 with the loads up front
-        int c = cp;
-        for (; c + 3 * parts < DW; c += 4 * parts) {
-          float kv[4];
-#pragma unroll
-          for (int u = 0; u < 4; ++u) kv[u] = kq[(size_t)(c + u * parts) * p.Mp];
-#pragma unroll
-          for (int u = 0; u < 4; ++u) {
-            const int cc = c + u * parts;
-            const uint64_t kk = pack2(kv[u], kv[u]);
-#pragma unroll
-            for (int rq = 0; rq < 4; ++rq) {
-              const float4 q4 = *reinterpret_cast<const float4 *>(qq + cc * kSelRowsMax + ((rq ^ (cc & 3)) << 2));
-              acc[2 * rq] = fma2(pack2(q4.x, q4.y), kk, acc[2 * rq]);
-              acc[2 * rq + 1] = fma2(pack2(q4.z, q4.w), kk, acc[2 * rq + 1]);
-            }
-          }
-        }
-        for (; c < DW; c += parts) {
-          const float kv = kq[(size_t)c * p.Mp];
-          const uint64_t kk = pack2(kv, kv);
-#pragma unroll
-          for (int rq = 0; rq < 4; ++rq) {
-            const float4 q4 = *reinterpret_cast<const float4 *>(qq + c * kSelRowsMax + ((rq ^ (c & 3)) << 2));
-            acc[2 * rq] = fma2(pack2(q4.x, q4.y), kk, acc[2 * rq]);
-            acc[2 * rq + 1] = fma2(pack2(q4.z, q4.w), kk, acc[2 * rq + 1]);
-          }
+        switch (nrq) {                                     // CTA-uniform: only the row quads this CTA holds
+          case 1: score_quarter<1>(kq, qq, cp, parts, DW, p.Mp, acc); break;
+          case 2: score_quarter<2>(kq, qq, cp, parts, DW, p.Mp, acc); break;
+          case 3: score_quarter<3>(kq, qq, cp, parts, DW, p.Mp, acc); break;
+          default: score_quarter<4>(kq, qq, cp, parts, DW, p.Mp, acc); break;
         }
       }
       if (q + n_slots < 4) {                               // the ring is shorter than the head: refill the slot just read
@@ -267,12 +293,15 @@ __global__ void __launch_bounds__(kSelWarps * 32) li_score_topk_kernel(const Sel
       }
     }
     if (cp < parts && g < nx) {
+      float *pw = part + (size_t)cp * kSelRowsMax * p.Mp + 32 * g + lane;
 #pragma unroll
       for (int rp = 0; rp < kSelRowsMax / 2; ++rp) {
-        float s0, s1;
-        unpack2(acc[rp], s0, s1);
-        part[((size_t)cp * kSelRowsMax + 2 * rp) * p.Mp + 32 * g + lane] = s0;
-        part[((size_t)cp * kSelRowsMax + 2 * rp + 1) * p.Mp + 32 * g + lane] = s1;
+        if (2 * rp < R) {                                  // CTA-uniform
+          float s0, s1;
+          unpack2(acc[rp], s0, s1);
+          pw[(size_t)(2 * rp) * p.Mp] = s0;
+          pw[(size_t)(2 * rp + 1) * p.Mp] = s1;
+        }
       }
     }
   }
@@ -283,28 +312,46 @@ __global__ void __launch_bounds__(kSelWarps * 32) li_score_topk_kernel(const Sel
   int32_t *out = p.sel_idx + row * p.kmax;
   if (lane == 0) p.sel_cnt[row] = k;
   uint32_t kr[NX];
+  {
+    // a score = its channel parts added in a fixed order (part 0 first)
+    float dot[NX];
+    const float *pr = part + (size_t)warp * p.Mp + lane;
 #pragma unroll
-  for (int x = 0; x < NX; ++x) {
-    const int m = lane + 32 * x;
-    kr[x] = 0u;                                            // absent blocks: key 0, below every real key
-    if (m < M && scoring) {
-      float dot = part[(size_t)warp * p.Mp + m];
-      for (int pp = 1; pp < parts; ++pp) dot += part[((size_t)pp * kSelRowsMax + warp) * p.Mp + m];   // fixed order
-      const float sv = dot * p.inv_sqrt_d + 0.0f;          // -0 -> +0 so that equal scores have equal keys
-      kr[x] = order_key(sv);
-      if (p.scores != nullptr) p.scores[row * p.score_pitch + m] = sv;
+    for (int x = 0; x < NX; ++x) dot[x] = (lane + 32 * x < M && scoring) ? pr[32 * x] : 0.f;
+    for (int pp = 1; pp < parts; ++pp) {
+      pr += (size_t)kSelRowsMax * p.Mp;
+#pragma unroll
+      for (int x = 0; x < NX; ++x)
+        if (lane + 32 * x < M && scoring) dot[x] += pr[32 * x];
+    }
+#pragma unroll
+    for (int x = 0; x < NX; ++x) {
+      const int m = lane + 32 * x;
+      kr[x] = 0u;                                          // absent blocks: key 0, below every real key
+      if (m < M && scoring) {
+        const float sv = dot[x] * p.inv_sqrt_d + 0.0f;     // -0 -> +0 so that equal scores have equal keys
+        kr[x] = order_key(sv);
+        if (p.scores != nullptr) p.scores[row * p.score_pitch + m] = sv;
+      }
     }
   }
   if (k > 0) {
     // T = k-th largest key: built MSB first, keeping count(key >= T) >= k
+    // (the search ends as soon as exactly k keys are >= T: that set is the answer, whatever the lower bits of the k-th)
     uint32_t T = 0;
     for (int bit = 31; bit >= 0; --bit) {
       const uint32_t cand = T | (1u << bit);
-      int c = 0;
+      int c0 = 0, c1 = 0;
 #pragma unroll
-      for (int x = 0; x < NX; ++x) c += kr[x] >= cand;
-      c = __reduce_add_sync(0xffffffffu, c);
-      if (c >= k) T = cand;
+      for (int x = 0; x < NX; x += 2) {
+        c0 += kr[x] >= cand;
+        if (x + 1 < NX) c1 += kr[x + 1] >= cand;
+      }
+      const int c = __reduce_add_sync(0xffffffffu, c0 + c1);
+      if (c >= k) {
+        T = cand;
+        if (c == k) break;                                 // warp-uniform
+      }
     }
     int c_gt = 0;
 #pragma unroll
@@ -481,15 +528,9 @@ int launch_pool_pages(const SelectParams &sp, const int32_t *pages, int n_list, 
 }
 
 constexpr size_t kSelSmemMax = 227 * 1024;
-template <int D, int NX>
-static cudaError_t launch_score_topk_nx(cudaLaunchConfig_t &cfg, const SelectParams &sp, const BatchMeta &meta) {
-  // rows per CTA: the fewest CTAs per head whose rows fit 16 warps, rows spread evenly (49 rows -> 4 CTAs of 13, 13, 13, 10)
-  const int groups = (sp.Nqb + kSelRowsMax - 1) / kSelRowsMax, rows = (sp.Nqb + groups - 1) / groups;
-  int n_slots = 4;                                         // channel quarters of kbar[bh] resident at once (2 always fit)
-  while (n_slots > 1 && sel_smem_bytes(D, sp.Mp, n_slots) > kSelSmemMax) --n_slots;
-  cfg.gridDim = dim3(groups, sp.B * sp.H);
-  cfg.blockDim = dim3(kSelWarps * 32);
-  cfg.dynamicSmemBytes = sel_smem_bytes(D, sp.Mp, n_slots);
+template <int D, int NX, int MINB>
+static cudaError_t launch_score_topk_inst(cudaLaunchConfig_t &cfg, const SelectParams &sp, const BatchMeta &meta, int rows,
+                                          int n_slots) {
   if (cfg.dynamicSmemBytes > 48 * 1024) {                  // above 48 KB the limit is raised once per device
     static std::atomic<uint64_t> attr_done{0};
     int dev = 0;
@@ -497,12 +538,30 @@ static cudaError_t launch_score_topk_nx(cudaLaunchConfig_t &cfg, const SelectPar
     if (e != cudaSuccess) return e;
     const uint64_t dev_bit = 1ull << (dev & 63);
     if (!(attr_done.load(std::memory_order_acquire) & dev_bit)) {
-      e = cudaFuncSetAttribute(li_score_topk_kernel<D, NX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSelSmemMax);
+      e = cudaFuncSetAttribute(li_score_topk_kernel<D, NX, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSelSmemMax);
       if (e != cudaSuccess) return e;
       attr_done.fetch_or(dev_bit, std::memory_order_release);
     }
   }
-  return cudaLaunchKernelEx(&cfg, li_score_topk_kernel<D, NX>, sp, meta, rows, n_slots);
+  return cudaLaunchKernelEx(&cfg, li_score_topk_kernel<D, NX, MINB>, sp, meta, rows, n_slots);
+}
+template <int D, int NX>
+static cudaError_t launch_score_topk_nx(cudaLaunchConfig_t &cfg, const SelectParams &sp, const BatchMeta &meta) {
+  // rows per CTA: at least the fewest CTAs per head whose rows fit 16 warps; more while the grid stays inside one wave of
+  // one CTA per SM (phase 1 costs a CTA per row QUAD it holds, phase 2 runs one warp per row), rows spread evenly:
+  // 49 rows x 24 heads on 148 SMs -> 6 CTAs per head of 9, 9, 9, 9, 9, 4 rows (3 quads) instead of 4 of 13 (4 quads)
+  int groups = (sp.Nqb + kSelRowsMax - 1) / kSelRowsMax;
+  const int n_sm = device_sm_count(), per_wave = n_sm / (sp.B * sp.H);
+  if (per_wave > groups) groups = per_wave < sp.Nqb ? per_wave : sp.Nqb;
+  const int rows = (sp.Nqb + groups - 1) / groups;
+  groups = (sp.Nqb + rows - 1) / rows;
+  int n_slots = 4;                                         // channel quarters of kbar[bh] resident at once (2 always fit)
+  while (n_slots > 1 && sel_smem_bytes(D, sp.Mp, n_slots) > kSelSmemMax) --n_slots;
+  cfg.gridDim = dim3(groups, sp.B * sp.H);
+  cfg.blockDim = dim3(kSelWarps * 32);
+  cfg.dynamicSmemBytes = sel_smem_bytes(D, sp.Mp, n_slots);
+  if (groups * sp.B * sp.H <= n_sm) return launch_score_topk_inst<D, NX, 1>(cfg, sp, meta, rows, n_slots);
+  return launch_score_topk_inst<D, NX, 2>(cfg, sp, meta, rows, n_slots);
 }
 template <int D>
 static cudaError_t launch_score_topk(cudaLaunchConfig_t &cfg, const SelectParams &sp, const BatchMeta &meta) {
