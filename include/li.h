@@ -46,8 +46,9 @@ enum {
   LI_ERR_INVALID_ARG = -1,      /* NULL pointer, non-positive size, bad stride/alignment, bad frame list */
   LI_ERR_UNSUPPORTED = -2,      /* d not in {64,128}; block not in {64,128}; block_q != block_k; B > LI_MAX_CALLS */
   LI_ERR_WORKSPACE   = -3,      /* workspace NULL or smaller than li_workspace_bytes() */
-  LI_ERR_CUDA        = -4       /* a CUDA runtime/driver call failed (no device, launch error, ...); the runtime's own
+  LI_ERR_CUDA        = -4,      /* a CUDA runtime/driver call failed (no device, launch error, ...); the runtime's own
                                    code is returned by li_last_cuda_error() */
+  LI_ERR_TOO_LARGE   = -5       /* li_block_select_static: the problem needs more than LI_STATIC_SCRATCH_BYTES of scratch */
 };
 
 /* li_problem.flags */
@@ -119,6 +120,27 @@ int li_block_select(const li_problem *p, const int32_t *top_k_host, int32_t kmax
 int li_block_select_reuse_kbar(const li_problem *p, const int32_t *top_k_host, int32_t kmax,
                                int32_t *sel_idx, int32_t *sel_cnt, float *scores_opt, int32_t score_pitch,
                                void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* li_block_select for callers that cannot allocate device memory (code under CUDA graph capture, serving loops and
+ * harnesses that forbid cudaMalloc): same operation, same arguments, same results bit for bit (Eq. 9-10,
+ * PAPER.md:131-140), but the scratch (pooled means qbar / kbar, and the score keys of the M > 512 path) lives in a
+ * file-scope __device__ array of LI_STATIC_SCRATCH_BYTES inside libli.so instead of a caller-supplied workspace.  The
+ * call allocates nothing (no cudaMalloc / cudaFree, no allocating library routine); every GPU that loads the library
+ * holds the array until the process exits.
+ *   - A problem whose select scratch, align256(B*H*Nqb*d*4) + align256(B*H*Mp*d*4) + align256(B*H*Nqb*max(Mmax,1)*4)
+ *     bytes (Mp = Mmax rounded up to 32; li_static_scratch_needed() returns it), exceeds LI_STATIC_SCRATCH_BYTES is
+ *     rejected with LI_ERR_TOO_LARGE before anything is launched (`mid` needs 3.7 MB, `long` 7.5 MB).
+ *   - ALL calls on a device share the one array, and it keeps the previous call's contents.  Nothing in it has to start
+ *     at zero: every value a call reads it has written itself (padding columns of kbar are copied but never used).
+ *     Calls that may overlap on the GPU (different streams, no ordering between them) RACE on it: order them, or give
+ *     the overlapping ones their own workspace through li_block_select.
+ *   - The pooled keys are not kept for li_block_select_reuse_kbar (that call takes the caller's workspace). */
+#define LI_STATIC_SCRATCH_BYTES (16u << 20)
+int li_block_select_static(const li_problem *p, const int32_t *top_k_host, int32_t kmax,
+                           int32_t *sel_idx, int32_t *sel_cnt, float *scores_opt, int32_t score_pitch,
+                           void *cuda_stream);
+/* Bytes of the array the call above would use for problem p (0 on invalid p); no device is touched. */
+size_t li_static_scratch_needed(const li_problem *p);
 
 /* Page-resident pooled slices (3-D tiling only; LI_ERR_UNSUPPORTED otherwise).  A 3-D block is bt frames
  * x one bh x bw patch of the frame grid, and the sum of a frame's K rows over a patch does not depend on where the frame

@@ -16,13 +16,15 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libli.so")
 
-LI_OK, LI_ERR_INVALID_ARG, LI_ERR_UNSUPPORTED, LI_ERR_WORKSPACE, LI_ERR_CUDA = 0, -1, -2, -3, -4
+LI_OK, LI_ERR_INVALID_ARG, LI_ERR_UNSUPPORTED, LI_ERR_WORKSPACE, LI_ERR_CUDA, LI_ERR_TOO_LARGE = 0, -1, -2, -3, -4, -5
+LI_STATIC_SCRATCH_BYTES = 16 << 20
 LI_MAX_CALLS = 64
 LI_FLAG_NO_SPLIT = 1
 LI_FLAG_KV_FP8 = 2
 LI_BAD_PAGE_ID, LI_BAD_SEL_CNT, LI_BAD_SEL_RANGE, LI_BAD_SEL_DUPLICATE = 1, 2, 4, 8
 
-EXPORTS = ("li_block_select", "li_block_select_reuse_kbar", "li_block_select_cached", "li_pool_pages", "li_slice_cache_bytes",
+EXPORTS = ("li_block_select", "li_block_select_reuse_kbar", "li_block_select_cached", "li_block_select_static",
+           "li_static_scratch_needed", "li_pool_pages", "li_slice_cache_bytes",
            "li_sparse_attn", "li_validate", "li_quantize_pages", "li_workspace_bytes", "li_context_policy",
            "li_policy_workspace_bytes", "li_launch_count", "li_reset_launch_count", "li_strerror", "li_version",
            "li_last_cuda_error")
@@ -94,6 +96,11 @@ def lib() -> ctypes.CDLL:
                                       ctypes.c_void_p]
         L.li_block_select_reuse_kbar.restype = ctypes.c_int
         L.li_block_select_reuse_kbar.argtypes = L.li_block_select.argtypes
+        L.li_block_select_static.restype = ctypes.c_int
+        L.li_block_select_static.argtypes = [P, ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p, ctypes.c_void_p,
+                                             ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p]
+        L.li_static_scratch_needed.restype = ctypes.c_size_t
+        L.li_static_scratch_needed.argtypes = [P]
         L.li_sparse_attn.restype = ctypes.c_int
         L.li_sparse_attn.argtypes = [P, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p,
                                      ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p]
@@ -241,6 +248,24 @@ def li_block_select(ctx: Context, top_k: Sequence[int], kmax: int, sel_idx: torc
                                _stream_ptr(stream))
     if rc != LI_OK:
         raise LiError(rc, "li_block_select")
+
+
+def li_block_select_static(ctx: Context, top_k: Sequence[int], kmax: int, sel_idx: torch.Tensor, sel_cnt: torch.Tensor,
+                           scores: Optional[torch.Tensor] = None, stream: Optional[torch.cuda.Stream] = None) -> None:
+    """li_block_select_static (include/li.h): li_block_select without a workspace argument and without any allocation; the
+    scratch is a LI_STATIC_SCRATCH_BYTES array inside libli.so shared by all calls (LiError LI_ERR_TOO_LARGE beyond it)."""
+    tk = np.ascontiguousarray(np.asarray(top_k, dtype=np.int32))
+    if len(tk) != ctx.B:
+        raise ValueError("top_k must have B entries")
+    pitch = int(scores.shape[-1]) if scores is not None else 0
+    rc = lib().li_block_select_static(ctypes.byref(ctx.p), tk.ctypes.data, int(kmax), sel_idx.data_ptr(), sel_cnt.data_ptr(),
+                                      scores.data_ptr() if scores is not None else None, pitch, _stream_ptr(stream))
+    if rc != LI_OK:
+        raise LiError(rc, "li_block_select_static")
+
+
+def li_static_scratch_needed(ctx: Context) -> int:
+    return int(lib().li_static_scratch_needed(ctypes.byref(ctx.p)))
 
 
 def li_slice_cache_bytes(ctx: Context) -> int:

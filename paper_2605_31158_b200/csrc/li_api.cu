@@ -327,6 +327,51 @@ int li_block_select_reuse_kbar(const li_problem *p, const int32_t *top_k_host, i
                            cuda_stream, 1);
 }
 
+// ----------------------------------------------------------------------------- li_block_select_static (include/li.h)
+// Scratch of the no-allocation entry point: one array per device that loads the library, shared by every call, never
+// cleared (a call reads only what it has written).  In host code the NAME g_static_scratch is a host-side stand-in, not
+// a device address; the address the kernels get is looked up once per device with cudaGetSymbolAddress.
+static __device__ __align__(256) unsigned char g_static_scratch[LI_STATIC_SCRATCH_BYTES];
+
+static int static_scratch_ptr(void **out) {
+  static std::atomic<void *> dev_ptr[64];                  // per device ordinal, resolved with that device current
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return (int)e;
+  if (dev < 0 || dev >= 64) return (int)cudaErrorInvalidDevice;
+  void *ptr = dev_ptr[dev].load(std::memory_order_acquire);
+  if (ptr == nullptr) {
+    e = cudaGetSymbolAddress(&ptr, g_static_scratch);
+    if (e != cudaSuccess) return (int)e;
+    if (ptr == nullptr || ((uintptr_t)ptr & 255u)) return (int)cudaErrorInvalidSymbol;
+    dev_ptr[dev].store(ptr, std::memory_order_release);
+  }
+  *out = ptr;
+  return 0;
+}
+
+size_t li_static_scratch_needed(const li_problem *p) {
+  Derived dv;
+  if (check_problem(p, &dv) != LI_OK) return 0;
+  return ws_bytes(p, dv);
+}
+
+int li_block_select_static(const li_problem *p, const int32_t *top_k_host, int32_t kmax, int32_t *sel_idx,
+                           int32_t *sel_cnt, float *scores_opt, int32_t score_pitch, void *cuda_stream) {
+  Derived dv;
+  const int rc = check_problem(p, &dv);
+  if (rc != LI_OK) return rc;
+  const size_t need = ws_bytes(p, dv);                     // what li_block_select touches of its workspace
+  if (need > (size_t)LI_STATIC_SCRATCH_BYTES) return LI_ERR_TOO_LARGE;
+  void *scratch = nullptr;
+  const int e = static_scratch_ptr(&scratch);
+  if (e != 0) return cuda_failed(e);
+  // block_select_impl asks for the full li_workspace_bytes (select region + the attention kernel's split region behind
+  // it) but reads and writes the select region only, which `need` bounds: the size passed is that requirement
+  return block_select_impl(p, top_k_host, kmax, sel_idx, sel_cnt, scores_opt, score_pitch, scratch,
+                           need + ws_split_bytes(p), cuda_stream, 0);
+}
+
 int li_sparse_attn(const li_problem *p, const int32_t *sel_idx, const int32_t *sel_cnt, int32_t kmax, void *o,
                    float *lse_opt, void *workspace, size_t workspace_bytes, void *cuda_stream) {
   Derived dv;
@@ -468,6 +513,7 @@ const char *li_strerror(int code) {
     case LI_ERR_UNSUPPORTED: return "unsupported configuration";
     case LI_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
     case LI_ERR_CUDA: return "CUDA error";
+    case LI_ERR_TOO_LARGE: return "problem needs more scratch than LI_STATIC_SCRATCH_BYTES (use li_block_select with a workspace)";
     default: return "unknown error";
   }
 }
