@@ -330,6 +330,35 @@ def test_whole_step_is_cuda_graph_capturable(P):
         assert torch.equal(buf.sel_idx, sel) and torch.equal(buf.o, o) and torch.equal(buf.lse, lse)
 
 
+def test_calls_on_two_streams_overlap_without_interference(P):
+    """include/li.h: calls share no state beyond what the caller passes (own workspace, own outputs).  Two different
+    problems are issued alternately on two streams, many times, so that their kernels overlap on the GPU (both grids are
+    far below one wave, both take the key-range split and its merge buffers in their OWN workspace); every result must
+    equal the one the same call gives when run alone."""
+    import paper_2605_31158_b200 as li
+    specs = [W.spec_small(name="conc-a", H=2, d=128, block=128, frame_tokens=200, n_cur_frames=3, n_pages=24,
+                          n_mem=(6,), n_win=(14,), density=Fraction(1, 2)),
+             W.spec_small(name="conc-b", seed=7117, H=3, d=64, block=64, frame_tokens=72, n_cur_frames=3, n_pages=48,
+                          n_mem=(12,), n_win=(28,), density=Fraction(1, 3))]
+    probs = [W.build(sp) for sp in specs]
+    runs = [P.run_gpu(pr, want_scores=False) for pr in probs]          # alone, on the current stream
+    refs = [(b.sel_idx.clone(), b.sel_cnt.clone(), b.o.clone(), b.lse.clone()) for _, b in runs]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    for s_ in streams:
+        s_.wait_stream(torch.cuda.current_stream())
+    for rep in range(20):
+        for (ctx, buf), pr, s_ in zip(runs, probs, streams):
+            with torch.cuda.stream(s_):
+                buf.sel_idx.fill_(-9)
+                buf.o.zero_()
+                li.forward(ctx, pr.top_k, buf, stream=s_)
+        torch.cuda.synchronize()
+        for (ctx, buf), ref in zip(runs, refs):
+            assert torch.equal(buf.sel_idx, ref[0]) and torch.equal(buf.sel_cnt, ref[1]), f"rep {rep}: mask differs"
+            assert torch.equal(buf.o.view(torch.int16), ref[2].view(torch.int16)), f"rep {rep}: O differs"
+            assert torch.equal(buf.lse.view(torch.int32), ref[3].view(torch.int32))
+
+
 @pytest.mark.parametrize("d,block", [(64, 64), (128, 64), (64, 128)])
 def test_tail_wave_split_other_tile_shapes(P, d, block):
     """The split instances of the other (d, block) template variants: 64-key blocks (32-key half-tiles) and d = 64."""
