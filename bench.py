@@ -543,6 +543,9 @@ def run_cuda(args):
             "gpu_launches": int(launches), "clocks": clk.summary(),
         }
         line.update(extras)
+        if "step_ms_sustained" in extras:
+            # the long run against the SUSTAINED peak (the kernel is timed inside a long step there): whole step, select included
+            line["step_sustained_frac_of_sustained_peak"] = flops / (extras["step_ms_sustained"] * 1e-3) / 1e12 / pk["bf16_tflops_sustained"]
         if not args.no_cpu and world == 1 and not fp8:
             dt, fl, desc = oracle_sample(prob, args.ref_heads, args.ref_tiles)
             line["cpu_baseline"] = {"value": fl / dt / 1e12, "unit": UNIT, "cores": cpu_threads(), "kind": "oracle",
