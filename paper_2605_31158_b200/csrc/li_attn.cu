@@ -17,7 +17,8 @@
 // buffer once S has been read), [128,128+D) O.
 // On B200 this kernel runs into the 1 kW power cap (SM clock ~1.6 GHz under load); DESIGN.md section 6.3 lists the
 // measured alternatives (one CTA per SM with Q in tensor memory, two softmax groups, FMA-pipe exp2, full-tile QK,
-// speculative / prefetching softmax loop, ...).
+// speculative / prefetching softmax loop, ...).  The TMEM budget above is what fixes the design: the one measured
+// gain left (QK with Q as a tensor-memory A operand, -5.7 %) needs 64 more columns than two co-resident CTAs have.
 // KV8 instances (LI_FLAG_KV_FP8): K/V pages hold e4m3 codes; the softmax warps first turn the bf16 Q
 // tile into its per-row e4m3 image in shared memory, both contractions run on tcgen05.mma.kind::f8f6f4 and P is
 // rounded to e4m3 (four keys per TMEM column).
